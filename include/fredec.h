@@ -1,0 +1,138 @@
+/*
+ * fredec.h -- C-ABI of libfredec_b200.so: the single-frequency (residual) periodogram
+ * scan of FREDEC (Baluev 2013, arXiv:1309.0100) on one NVIDIA B200 (sm_100a).
+ *
+ * Citations "PAPER.md:NNN" are line numbers of the paper text this build was written
+ * from; "DESIGN.md Sx/Gx" are this build's readings of points the paper leaves open.
+ *
+ * Notation (section 2): a time series of N times t_i, measurements x_i and
+ * weights w_i; <phi> = sum_i w_i phi(t_i) (eq. 3); chi2 = <(x - mu)^2>
+ * (eq. 4).  The base model is mu_base(t) = sum_{j<d} theta_j phi_j(t), given by
+ * the VALUES of its d functions on the times (a constant, eq. 1; a polynomial,
+ * PAPER.md:51; constant + accepted sinusoids, eq. 2).  The trial model adds
+ * a cos(2 pi f t) + b sin(2 pi f t) with f fixed and all d+2 linear coefficients fitted
+ * exactly (eq. 5; eq. 10 with n = 1).
+ *
+ * Conventions for every entry point
+ *   - All floating-point arrays are IEEE double, all indices int64_t, row-major, dense.
+ *   - Every data pointer may be a HOST pointer or a CUDA DEVICE pointer (of the current
+ *     device); the library classifies each one with cudaPointerGetAttributes.  Host
+ *     buffers are staged through library-owned device memory; device buffers are used in
+ *     place (this is the measured path).  Inputs are never modified.
+ *   - The caller owns every buffer it passes; the library keeps no pointer after return.
+ *     Internal workspace is library-owned, grows lazily and is freed by fredec_shutdown().
+ *   - Work is enqueued on the stream set by fredec_set_stream() (default: the legacy
+ *     default stream).  Every compute entry point returns AFTER its work has completed on
+ *     that stream, so that the returned status is final and outputs are ready.
+ *   - Return value: FREDEC_OK (0) or a count >= 0 on success, a negative FREDEC_E* code
+ *     on failure.  Nothing throws, aborts or prints.  On failure outputs are unspecified.
+ *   - There is NO CPU fallback: without a usable CUDA device compute calls return
+ *     FREDEC_ECUDA.
+ *   - Not thread-safe: one caller at a time per process (one process per GPU).
+ */
+#ifndef FREDEC_H
+#define FREDEC_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FREDEC_OK 0
+#define FREDEC_EINVAL (-1)    /* NULL required pointer, N < d+3, d < 0 or d > FREDEC_D_MAX, B < 1, K < 1,
+                                 k < 1, k > K or k > FREDEC_TOPK_MAX, df <= 0, f0 < 0, non-finite f0/df */
+#define FREDEC_EDATA (-2)     /* non-finite t/x/w/base value, w_i < 0, sum w = 0 */
+#define FREDEC_ESINGULAR (-3) /* base functions linearly dependent (S6b) */
+#define FREDEC_ECUDA (-4)     /* CUDA runtime error; see fredec_last_cuda_error() */
+
+#define FREDEC_D_MAX 64       /* the paper's pools reach n = 25 sinusoids => d = 51 */
+#define FREDEC_TOPK_MAX 1024
+
+/*
+ * fredec_scan -- periodogram scan (section 4.2 "single-frequency residual
+ * periodograms"; eq. 10; sums of PAPER.md:165-171 eqs. 15-16; solve of
+ * PAPER.md:175).  For k = 0..K-1, with f_k = f0 + k*df (cycles per unit of t):
+ *
+ *   z_out[k] = min_theta chi2(base)  -  min_{theta,a,b} chi2(base + a cos 2 pi f_k t + b sin 2 pi f_k t)
+ *
+ * i.e. the chi-square reduction, in the units of sum w x^2; 0 <= z_out[k] <= chi2_base.
+ * The paper's statistic is the monotone transform z = (N_H/2) ln(chi2_base/(chi2_base - z_out))
+ * (eq. 8, reading G1), so peak positions are identical.
+ *
+ *   t, x, w      [N]     times, measurements, weights (w_i >= 0); any order of t
+ *   N                    number of observations, N >= d + 3 (N_H = N - 3n - 1 > 0)
+ *   base_funcs   [d][N]  values phi_j(t_i) of the base-model functions; NULL allowed iff d == 0
+ *   d                    0 <= d <= FREDEC_D_MAX
+ *   f0, df, K            frequency grid, f0 >= 0, df > 0, K >= 1 ("dense enough ... grid")
+ *   z_out        [K]     output
+ *
+ * A trial frequency whose cos/sin column lies in the span of the base (f = 0 with a constant
+ * in the base; f equal to a base frequency) contributes nothing: that column is dropped and
+ * z stays finite (reading S6).  Never writes NaN or inf.
+ */
+int fredec_scan(const double* t, const double* x, const double* w, int64_t N,
+                const double* base_funcs, int32_t d,
+                double f0, double df, int64_t K, double* z_out);
+
+/*
+ * fredec_scan_batched -- B independent series of equal length on a shared grid.
+ *   t, x, w [B][N];  base_funcs [B][d][N];  z_out [B][K].
+ */
+int fredec_scan_batched(const double* t, const double* x, const double* w, int64_t B, int64_t N,
+                        const double* base_funcs, int32_t d,
+                        double f0, double df, int64_t K, double* z_out);
+
+/*
+ * fredec_chi2_base -- chi2_base = min_theta <(x - sum_j theta_j phi_j)^2>, the l_m of
+ * PAPER.md:81 (eq. 7) for the base model alone; upper bound of z_out and the quantity the
+ * paper's statistic normalises by.  Arguments as fredec_scan; chi2_base_out is one double
+ * ([B] doubles for the batched form).
+ */
+int fredec_chi2_base(const double* t, const double* x, const double* w, int64_t N,
+                     const double* base_funcs, int32_t d, double* chi2_base_out);
+int fredec_chi2_base_batched(const double* t, const double* x, const double* w, int64_t B, int64_t N,
+                             const double* base_funcs, int32_t d, double* chi2_base_out);
+
+/*
+ * fredec_topk -- peak extraction on a periodogram ("the largest peak
+ * remaining" and the "other periodogram peaks").  Reading S7: index i is a peak iff
+ * z[i] > z[i-1] and z[i] >= z[i+1] (a plateau yields its lowest index); neighbours outside
+ * [0, K) and NaN count as -infinity.  Peaks are ranked by z descending, then index ascending;
+ * the first k indices go to idx_out[0..k-1]; unused slots are -1.  Bit-exact in indices.
+ * Returns the number of peaks written (0..k), or a negative error code.
+ *   z [K] input;  1 <= k <= min(K, FREDEC_TOPK_MAX);  idx_out [k].
+ * Batched form: z [B][K], idx_out [B][k]; returns FREDEC_OK.
+ */
+int fredec_topk(const double* z, int64_t K, int32_t k, int64_t* idx_out);
+int fredec_topk_batched(const double* z, int64_t B, int64_t K, int32_t k, int64_t* idx_out);
+
+/* ----------------------------------------------------------------- runtime control */
+
+/* Stream on which all work is enqueued (a cudaStream_t passed as void*); NULL = default. */
+int fredec_set_stream(void* cuda_stream);
+
+/* Device-side durations (ms, CUDA events on the library's stream) of the kernels of the LAST
+ * compute call: out[0] = base orthogonalisation + packing kernel(s), out[1] = scan kernel(s),
+ * out[2] = top-k kernel(s), out[3] = whole call including staging copies. Unused = 0. */
+int fredec_last_timing(double out[4]);
+
+/* Number of kernels the LAST compute call launched. */
+int fredec_last_launches(void);
+
+/* Measures the FP64 FMA peak of the current device with a register-resident DFMA-only
+ * kernel on all SMs (roofline denominator, not part of the method).  iters = FMAs per
+ * thread per chain (>= 1024).  Outputs TFLOP/s (FMA = 2 flops) and kernel ms. */
+int fredec_fp64_peak(int64_t iters, double* tflops_out, double* ms_out);
+
+/* Frees all library-owned device memory, events and staging buffers. */
+int fredec_shutdown(void);
+
+const char* fredec_strerror(int code);
+int fredec_last_cuda_error(void);   /* the cudaError_t behind the last FREDEC_ECUDA, else 0 */
+int fredec_version(void);           /* 100*major + minor */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FREDEC_H */

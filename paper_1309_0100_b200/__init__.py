@@ -1,0 +1,12 @@
+"""B200-native periodogram scan of FREDEC (Baluev 2013, arXiv:1309.0100).
+
+The product is the C-ABI library libfredec_b200.so (include/fredec.h, sources under csrc/);
+this package is its thin Python binding plus the seeded input generators (`inputs`).
+"""
+from ._binding import (  # noqa: F401
+    FREDEC_D_MAX, FREDEC_ECUDA, FREDEC_EDATA, FREDEC_EINVAL, FREDEC_ESINGULAR, FREDEC_OK,
+    FREDEC_TOPK_MAX, FredecError, LIB_PATH,
+    fredec_chi2_base, fredec_chi2_base_batched, fredec_fp64_peak, fredec_last_launches,
+    fredec_last_timing, fredec_scan, fredec_scan_batched, fredec_set_stream, fredec_shutdown,
+    fredec_topk, fredec_topk_batched, fredec_version, lib,
+)

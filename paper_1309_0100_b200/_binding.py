@@ -1,0 +1,196 @@
+"""Thin ctypes binding of libfredec_b200.so (include/fredec.h): argument marshalling only.
+
+Every step of the scan runs in the CUDA kernels behind the C-ABI; nothing here computes.
+Arrays may be numpy arrays (host buffers, staged by the library) or torch tensors (CPU,
+pinned or CUDA; CUDA tensors are used in place).  There is no CPU fallback: a missing
+library or a failing CUDA call raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfredec_b200.so")
+
+FREDEC_OK, FREDEC_EINVAL, FREDEC_EDATA, FREDEC_ESINGULAR, FREDEC_ECUDA = 0, -1, -2, -3, -4
+FREDEC_D_MAX, FREDEC_TOPK_MAX = 64, 1024
+
+# name -> (restype, argtypes); must list every symbol include/fredec.h declares
+_P, _I64, _I32, _F64 = C.c_void_p, C.c_int64, C.c_int32, C.c_double
+SIGNATURES = {
+    "fredec_scan": (C.c_int, [_P, _P, _P, _I64, _P, _I32, _F64, _F64, _I64, _P]),
+    "fredec_scan_batched": (C.c_int, [_P, _P, _P, _I64, _I64, _P, _I32, _F64, _F64, _I64, _P]),
+    "fredec_chi2_base": (C.c_int, [_P, _P, _P, _I64, _P, _I32, _P]),
+    "fredec_chi2_base_batched": (C.c_int, [_P, _P, _P, _I64, _I64, _P, _I32, _P]),
+    "fredec_topk": (C.c_int, [_P, _I64, _I32, _P]),
+    "fredec_topk_batched": (C.c_int, [_P, _I64, _I64, _I32, _P]),
+    "fredec_set_stream": (C.c_int, [_P]),
+    "fredec_last_timing": (C.c_int, [C.POINTER(C.c_double)]),
+    "fredec_last_launches": (C.c_int, []),
+    "fredec_fp64_peak": (C.c_int, [_I64, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    "fredec_shutdown": (C.c_int, []),
+    "fredec_strerror": (C.c_char_p, [C.c_int]),
+    "fredec_last_cuda_error": (C.c_int, []),
+    "fredec_version": (C.c_int, []),
+}
+
+_lib = None
+
+
+class FredecError(RuntimeError):
+    def __init__(self, code: int, where: str, detail: str = ""):
+        self.code = code
+        super().__init__(f"{where} failed: {code} ({detail})")
+
+
+def lib():
+    """Loads libfredec_b200.so; raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_1309_0100_b200.build` "
+                "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, where: str) -> int:
+    if rc < 0:
+        L = lib()
+        detail = L.fredec_strerror(rc).decode()
+        if rc == FREDEC_ECUDA:
+            detail += f", cudaError {L.fredec_last_cuda_error()}"
+        raise FredecError(rc, where, detail)
+    return rc
+
+
+def _is_torch(a) -> bool:
+    return type(a).__module__.startswith("torch")
+
+
+def _ptr(a, dtype=np.float64):
+    """(address, keep-alive) of a contiguous float64/int64 numpy array or torch tensor."""
+    if a is None:
+        return None, None
+    if _is_torch(a):
+        import torch
+        want = torch.float64 if dtype == np.float64 else torch.int64
+        if a.dtype != want or not a.is_contiguous():
+            raise TypeError(f"need a contiguous {want} tensor")
+        return a.data_ptr(), a
+    arr = np.ascontiguousarray(a, dtype=dtype)
+    return arr.ctypes.data, arr
+
+
+def _empty_like_kind(ref, shape, dtype=np.float64):
+    if _is_torch(ref):
+        import torch
+        return torch.empty(shape, dtype=torch.float64 if dtype == np.float64 else torch.int64,
+                           device=ref.device)
+    return np.empty(shape, dtype=dtype)
+
+
+def fredec_set_stream(stream=None) -> None:
+    """stream: None (default stream), an int cudaStream_t, or a torch.cuda.Stream."""
+    handle = 0 if stream is None else getattr(stream, "cuda_stream", stream)
+    _check(lib().fredec_set_stream(C.c_void_p(int(handle))), "fredec_set_stream")
+
+
+def fredec_scan(t, x, w, base_funcs, f0, df, K, z_out=None):
+    """z[k] = chi-square reduction at f0 + k*df; see include/fredec.h."""
+    N = int(t.shape[-1])
+    d = 0 if base_funcs is None else int(base_funcs.shape[0]) if base_funcs.ndim == 2 else 1
+    if d == 0:
+        base_funcs = None
+    z = _empty_like_kind(t, (int(K),)) if z_out is None else z_out
+    (pt, kt), (px, kx), (pw, kw), (pb, kb), (pz, kz) = map(_ptr, (t, x, w, base_funcs, z))
+    _check(lib().fredec_scan(pt, px, pw, N, pb, d, float(f0), float(df), int(K), pz), "fredec_scan")
+    return z if z_out is None or kz is z else kz
+
+
+def fredec_scan_batched(t, x, w, base_funcs, f0, df, K, z_out=None):
+    B, N = int(t.shape[0]), int(t.shape[1])
+    d = 0 if base_funcs is None else int(base_funcs.shape[1])
+    if d == 0:
+        base_funcs = None
+    z = _empty_like_kind(t, (B, int(K))) if z_out is None else z_out
+    (pt, kt), (px, kx), (pw, kw), (pb, kb), (pz, kz) = map(_ptr, (t, x, w, base_funcs, z))
+    _check(lib().fredec_scan_batched(pt, px, pw, B, N, pb, d, float(f0), float(df), int(K), pz),
+           "fredec_scan_batched")
+    return z
+
+
+def fredec_chi2_base(t, x, w, base_funcs) -> float:
+    N = int(t.shape[-1])
+    d = 0 if base_funcs is None else int(base_funcs.shape[0])
+    if d == 0:
+        base_funcs = None
+    out = np.empty(1)
+    (pt, kt), (px, kx), (pw, kw), (pb, kb) = map(_ptr, (t, x, w, base_funcs))
+    _check(lib().fredec_chi2_base(pt, px, pw, N, pb, d, out.ctypes.data), "fredec_chi2_base")
+    return float(out[0])
+
+
+def fredec_chi2_base_batched(t, x, w, base_funcs):
+    B, N = int(t.shape[0]), int(t.shape[1])
+    d = 0 if base_funcs is None else int(base_funcs.shape[1])
+    if d == 0:
+        base_funcs = None
+    out = np.empty(B)
+    (pt, kt), (px, kx), (pw, kw), (pb, kb) = map(_ptr, (t, x, w, base_funcs))
+    _check(lib().fredec_chi2_base_batched(pt, px, pw, B, N, pb, d, out.ctypes.data),
+           "fredec_chi2_base_batched")
+    return out
+
+
+def fredec_topk(z, k, idx_out=None):
+    """Returns (idx[k], count): indices of the k highest peaks, -1 padded."""
+    K = int(z.shape[-1])
+    idx = _empty_like_kind(z, (int(k),), np.int64) if idx_out is None else idx_out
+    pz, kz = _ptr(z)
+    pi, ki = _ptr(idx, np.int64)
+    count = _check(lib().fredec_topk(pz, K, int(k), pi), "fredec_topk")
+    return idx, count
+
+
+def fredec_topk_batched(z, k, idx_out=None):
+    B, K = int(z.shape[0]), int(z.shape[1])
+    idx = _empty_like_kind(z, (B, int(k)), np.int64) if idx_out is None else idx_out
+    pz, kz = _ptr(z)
+    pi, ki = _ptr(idx, np.int64)
+    _check(lib().fredec_topk_batched(pz, B, K, int(k), pi), "fredec_topk_batched")
+    return idx
+
+
+def fredec_last_timing() -> dict:
+    out = (C.c_double * 4)()
+    _check(lib().fredec_last_timing(out), "fredec_last_timing")
+    return {"prep_ms": out[0], "scan_ms": out[1], "topk_ms": out[2], "total_ms": out[3]}
+
+
+def fredec_last_launches() -> int:
+    return int(lib().fredec_last_launches())
+
+
+def fredec_fp64_peak(iters: int = 1 << 16):
+    """(TFLOP/s, ms) of the DFMA-only microbenchmark: the FP64 roofline denominator."""
+    tf, ms = C.c_double(), C.c_double()
+    _check(lib().fredec_fp64_peak(int(iters), C.byref(tf), C.byref(ms)), "fredec_fp64_peak")
+    return tf.value, ms.value
+
+
+def fredec_shutdown() -> None:
+    _check(lib().fredec_shutdown(), "fredec_shutdown")
+
+
+def fredec_version() -> int:
+    return int(lib().fredec_version())

@@ -1,0 +1,452 @@
+// fredec_api.cu -- host side of libfredec_b200.so: the C-ABI of include/fredec.h.
+// Argument validation, host/device pointer staging, library-owned workspace, launch
+// configuration and device-side timing.  All arithmetic of the method runs in the kernels.
+#include <cmath>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <cuda_runtime.h>
+
+#include "fredec.h"
+#include "peak_kernel.cuh"
+#include "prep_kernel.cuh"
+#include "scan_kernel.cuh"
+#include "topk_kernel.cuh"
+
+using namespace fredec;
+
+namespace {
+
+struct DevBuf {
+    void* p = nullptr;
+    size_t cap = 0;
+    cudaError_t reserve(size_t n)
+    {
+        if (n <= cap) return cudaSuccess;
+        if (p) {
+            cudaError_t e = cudaFree(p);
+            p = nullptr;
+            cap = 0;
+            if (e != cudaSuccess) return e;
+        }
+        size_t want = n + n / 8 + 256;
+        cudaError_t e = cudaMalloc(&p, want);
+        if (e == cudaSuccess) cap = want;
+        return e;
+    }
+    void release()
+    {
+        if (p) cudaFree(p);
+        p = nullptr;
+        cap = 0;
+    }
+    template <class T>
+    T* as() const { return static_cast<T*>(p); }
+};
+
+struct HostBuf {
+    void* p = nullptr;
+    size_t cap = 0;
+    cudaError_t reserve(size_t n)
+    {
+        if (n <= cap) return cudaSuccess;
+        if (p) cudaFreeHost(p);
+        p = nullptr;
+        cap = 0;
+        cudaError_t e = cudaMallocHost(&p, n + 256);
+        if (e == cudaSuccess) cap = n + 256;
+        return e;
+    }
+    void release()
+    {
+        if (p) cudaFreeHost(p);
+        p = nullptr;
+        cap = 0;
+    }
+};
+
+constexpr int kNumEvents = 5;
+
+struct State {
+    bool ready = false;
+    int device = -1;
+    int sm_count = 0;
+    cudaStream_t stream = nullptr;
+    cudaEvent_t ev[kNumEvents] = {};
+    DevBuf in_t, in_x, in_w, in_base, in_z, out_z, out_idx, out_chi2;
+    DevBuf rec, psi, xt, info, ws, part_z, part_i, count, sink;
+    HostBuf h_info, h_count;
+    int last_cuda = 0;
+    double timing[4] = {0, 0, 0, 0};
+    int launches = 0;
+};
+State g;
+
+#define CK(expr)                                \
+    do {                                        \
+        cudaError_t e__ = (expr);               \
+        if (e__ != cudaSuccess) {               \
+            g.last_cuda = (int)e__;             \
+            (void)cudaGetLastError();           \
+            return FREDEC_ECUDA;                \
+        }                                       \
+    } while (0)
+
+int ensure_ready()
+{
+    if (g.ready) return FREDEC_OK;
+    int n = 0;
+    CK(cudaGetDeviceCount(&n));
+    if (n < 1) {
+        g.last_cuda = (int)cudaErrorNoDevice;
+        return FREDEC_ECUDA;
+    }
+    CK(cudaGetDevice(&g.device));
+    CK(cudaDeviceGetAttribute(&g.sm_count, cudaDevAttrMultiProcessorCount, g.device));
+    for (int i = 0; i < kNumEvents; ++i) CK(cudaEventCreate(&g.ev[i]));
+    g.ready = true;
+    return FREDEC_OK;
+}
+
+// true if p is usable from device code as is
+bool on_device(const void* p)
+{
+    cudaPointerAttributes a;
+    cudaError_t e = cudaPointerGetAttributes(&a, p);
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        return false;
+    }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+// device view of an input: the pointer itself, or a staged copy
+template <class T>
+int stage_in(const T* src, size_t count, DevBuf& buf, const T** out)
+{
+    if (src == nullptr || count == 0) {
+        *out = nullptr;
+        return FREDEC_OK;
+    }
+    if (on_device(src)) {
+        *out = src;
+        return FREDEC_OK;
+    }
+    CK(buf.reserve(count * sizeof(T)));
+    CK(cudaMemcpyAsync(buf.p, src, count * sizeof(T), cudaMemcpyHostToDevice, g.stream));
+    *out = buf.as<T>();
+    return FREDEC_OK;
+}
+
+// device view of an output; *host_dst != nullptr means "copy back to there afterwards"
+template <class T>
+int stage_out(T* dst, size_t count, DevBuf& buf, T** out, T** host_dst)
+{
+    if (on_device(dst)) {
+        *out = dst;
+        *host_dst = nullptr;
+        return FREDEC_OK;
+    }
+    CK(buf.reserve(count * sizeof(T)));
+    *out = buf.as<T>();
+    *host_dst = dst;
+    return FREDEC_OK;
+}
+
+struct ScanPlan {
+    int R, NB, n_pass, FW, S, TI;
+};
+
+ScanPlan plan_scan(int64_t B, int64_t N, int d, int64_t K)
+{
+    ScanPlan pl;
+    if (d <= 3) {
+        pl.R = 8; pl.NB = d; pl.n_pass = 1;
+    } else if (d <= 9) {
+        pl.R = 4; pl.NB = d; pl.n_pass = 1;
+    } else {
+        pl.R = 4; pl.NB = 8; pl.n_pass = (d + 7) / 8;
+    }
+    const int64_t runs = (K + pl.R - 1) / pl.R;
+    const int64_t fwarps = (runs + 31) / 32 * B;   // warps if every run had its own lane once
+    const int64_t target = (int64_t)g.sm_count * 8;
+    int S = 1;
+    while (S < 8 && fwarps * (S * 2) <= target && N / (S * 2) >= 16) S *= 2;
+    int FW = 1;
+    while (FW < 4 && FW * 2 * S <= 8 && fwarps / (FW * 2) >= 2 * (int64_t)g.sm_count) FW *= 2;
+    pl.S = S;
+    pl.FW = FW;
+    int TI = rec_stride(pl.NB) <= 16 ? 128 : 64;
+    if (N < TI) TI = (int)((N + S - 1) / S * S);
+    pl.TI = TI;
+    return pl;
+}
+
+int check_series_args(const double* t, const double* x, const double* w, int64_t B, int64_t N,
+                      const double* base_funcs, int32_t d)
+{
+    if (!t || !x || !w) return FREDEC_EINVAL;
+    if (B < 1 || d < 0 || d > FREDEC_D_MAX || N < (int64_t)d + 3) return FREDEC_EINVAL;
+    if (d > 0 && !base_funcs) return FREDEC_EINVAL;
+    if (B > 65535 || N > (int64_t)1 << 31) return FREDEC_EINVAL;
+    return FREDEC_OK;
+}
+
+float ev_ms(int a, int b)
+{
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, g.ev[a], g.ev[b]) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return 0.f;
+    }
+    return ms;
+}
+
+// Shared body of scan / chi2_base: with_scan == false runs only the prep kernel.
+int run_series(const double* t, const double* x, const double* w, int64_t B, int64_t N,
+               const double* base_funcs, int32_t d, double f0, double df, int64_t K,
+               double* z_out, double* chi2_out, bool with_scan)
+{
+    int rc = check_series_args(t, x, w, B, N, base_funcs, d);
+    if (rc) return rc;
+    if (with_scan) {
+        if (!z_out || K < 1 || !(df > 0.0) || !(f0 >= 0.0) || !std::isfinite(f0) || !std::isfinite(df))
+            return FREDEC_EINVAL;
+        if (!std::isfinite(f0 + df * (double)K)) return FREDEC_EINVAL;
+    } else if (!chi2_out) {
+        return FREDEC_EINVAL;
+    }
+    rc = ensure_ready();
+    if (rc) return rc;
+    g.launches = 0;
+    for (double& v : g.timing) v = 0.0;
+    cudaStream_t st = g.stream;
+
+    CK(cudaEventRecord(g.ev[0], st));
+    const double *dt, *dx, *dw, *dbase;
+    const size_t BN = (size_t)B * N;
+    if ((rc = stage_in(t, BN, g.in_t, &dt))) return rc;
+    if ((rc = stage_in(x, BN, g.in_x, &dx))) return rc;
+    if ((rc = stage_in(w, BN, g.in_w, &dw))) return rc;
+    if ((rc = stage_in(base_funcs, BN * d, g.in_base, &dbase))) return rc;
+
+    ScanPlan pl = plan_scan(B, N, d, with_scan ? K : 1);
+    const int RS = rec_stride(pl.NB);
+    CK(g.psi.reserve(BN * (size_t)(d > 0 ? d : 1) * 8));
+    CK(g.xt.reserve(BN * 8));
+    CK(g.info.reserve((size_t)B * sizeof(SeriesInfo)));
+    CK(g.h_info.reserve((size_t)B * sizeof(SeriesInfo)));
+    if (with_scan) CK(g.rec.reserve(BN * pl.n_pass * RS * 8));
+
+    PrepParams pp;
+    pp.t = dt; pp.x = dx; pp.w = dw; pp.base = dbase;
+    pp.psi = g.psi.as<double>(); pp.xt = g.xt.as<double>();
+    pp.rec = with_scan ? g.rec.as<double>() : nullptr;
+    pp.info = g.info.as<SeriesInfo>();
+    pp.N = N; pp.d = d; pp.NB = pl.NB; pp.n_pass = pl.n_pass; pp.R = pl.R; pp.df = with_scan ? df : 1.0;
+    CK(cudaEventRecord(g.ev[1], st));
+    CK(launch_prep(pp, B, st));
+    g.launches += 1;
+    CK(cudaEventRecord(g.ev[2], st));
+
+    double* dz = nullptr;
+    double* hz = nullptr;
+    if (with_scan) {
+        if ((rc = stage_out(z_out, (size_t)B * K, g.out_z, &dz, &hz))) return rc;
+        ScanParams sp;
+        sp.rec = g.rec.as<double>();
+        sp.info = g.info.as<SeriesInfo>();
+        sp.z = dz;
+        sp.N = N; sp.K = K;
+        const int64_t runs = (K + pl.R - 1) / pl.R;
+        sp.Kpad = runs * pl.R;
+        sp.f0 = f0; sp.df = df;
+        sp.n_pass = pl.n_pass;
+        sp.FW = pl.FW; sp.S = pl.S; sp.TI = pl.TI;
+        sp.ws = nullptr;
+        if (pl.n_pass > 1) {
+            CK(g.ws.reserve((size_t)B * 7 * sp.Kpad * 8));
+            sp.ws = g.ws.as<double>();
+        }
+        for (int pass = 0; pass < pl.n_pass; ++pass) {
+            sp.pass = pass;
+            CK(launch_scan(pl.R, pl.NB, sp, B, st));
+            g.launches += 1;
+        }
+    }
+    CK(cudaEventRecord(g.ev[3], st));
+    if (hz) CK(cudaMemcpyAsync(hz, dz, (size_t)B * K * 8, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(g.h_info.p, g.info.p, (size_t)B * sizeof(SeriesInfo), cudaMemcpyDeviceToHost, st));
+    CK(cudaEventRecord(g.ev[4], st));
+    CK(cudaStreamSynchronize(st));
+
+    g.timing[0] = ev_ms(1, 2);
+    g.timing[1] = ev_ms(2, 3);
+    g.timing[3] = ev_ms(0, 4);
+    const SeriesInfo* hi = static_cast<const SeriesInfo*>(g.h_info.p);
+    for (int64_t b = 0; b < B; ++b)
+        if (hi[b].status != 0) return hi[b].status;
+    if (chi2_out) {
+        if (on_device(chi2_out)) {
+            double* tmp = static_cast<double*>(std::malloc((size_t)B * 8));
+            if (!tmp) return FREDEC_EINVAL;
+            for (int64_t b = 0; b < B; ++b) tmp[b] = hi[b].chi2_base;
+            cudaError_t e = cudaMemcpy(chi2_out, tmp, (size_t)B * 8, cudaMemcpyHostToDevice);
+            std::free(tmp);
+            CK(e);
+        } else {
+            for (int64_t b = 0; b < B; ++b) chi2_out[b] = hi[b].chi2_base;
+        }
+    }
+    return FREDEC_OK;
+}
+
+int run_topk(const double* z, int64_t B, int64_t K, int32_t k, int64_t* idx_out, int* first_count)
+{
+    if (!z || !idx_out || B < 1 || B > 65535 || K < 1 || k < 1 || (int64_t)k > K || k > FREDEC_TOPK_MAX)
+        return FREDEC_EINVAL;
+    int rc = ensure_ready();
+    if (rc) return rc;
+    g.launches = 0;
+    for (double& v : g.timing) v = 0.0;
+    cudaStream_t st = g.stream;
+    CK(cudaEventRecord(g.ev[0], st));
+    const double* dz;
+    if ((rc = stage_in(z, (size_t)B * K, g.in_z, &dz))) return rc;
+    int64_t *didx, *hidx;
+    if ((rc = stage_out(idx_out, (size_t)B * k, g.out_idx, &didx, &hidx))) return rc;
+
+    TopkParams tp;
+    tp.z = dz; tp.idx_out = didx; tp.K = K; tp.k = k;
+    tp.nblk = topk_pick_nblk(B, K, g.sm_count);
+    CK(g.count.reserve((size_t)B * sizeof(int)));
+    CK(g.h_count.reserve((size_t)B * sizeof(int)));
+    tp.count_out = g.count.as<int>();
+    tp.part_z = nullptr; tp.part_i = nullptr;
+    if (tp.nblk > 1) {
+        CK(g.part_z.reserve((size_t)B * tp.nblk * k * 8));
+        CK(g.part_i.reserve((size_t)B * tp.nblk * k * 8));
+        tp.part_z = g.part_z.as<double>();
+        tp.part_i = g.part_i.as<int64_t>();
+    }
+    CK(cudaEventRecord(g.ev[1], st));
+    int nl = 0;
+    CK(launch_topk(tp, B, st, &nl));
+    g.launches = nl;
+    CK(cudaEventRecord(g.ev[3], st));
+    if (hidx) CK(cudaMemcpyAsync(hidx, didx, (size_t)B * k * 8, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(g.h_count.p, g.count.p, (size_t)B * sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaEventRecord(g.ev[4], st));
+    CK(cudaStreamSynchronize(st));
+    g.timing[2] = ev_ms(1, 3);
+    g.timing[3] = ev_ms(0, 4);
+    *first_count = static_cast<const int*>(g.h_count.p)[0];
+    return FREDEC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int fredec_scan(const double* t, const double* x, const double* w, int64_t N, const double* base_funcs,
+                int32_t d, double f0, double df, int64_t K, double* z_out)
+{
+    return run_series(t, x, w, 1, N, base_funcs, d, f0, df, K, z_out, nullptr, true);
+}
+
+int fredec_scan_batched(const double* t, const double* x, const double* w, int64_t B, int64_t N,
+                        const double* base_funcs, int32_t d, double f0, double df, int64_t K, double* z_out)
+{
+    return run_series(t, x, w, B, N, base_funcs, d, f0, df, K, z_out, nullptr, true);
+}
+
+int fredec_chi2_base(const double* t, const double* x, const double* w, int64_t N, const double* base_funcs,
+                     int32_t d, double* chi2_base_out)
+{
+    return run_series(t, x, w, 1, N, base_funcs, d, 0.0, 1.0, 1, nullptr, chi2_base_out, false);
+}
+
+int fredec_chi2_base_batched(const double* t, const double* x, const double* w, int64_t B, int64_t N,
+                             const double* base_funcs, int32_t d, double* chi2_base_out)
+{
+    return run_series(t, x, w, B, N, base_funcs, d, 0.0, 1.0, 1, nullptr, chi2_base_out, false);
+}
+
+int fredec_topk(const double* z, int64_t K, int32_t k, int64_t* idx_out)
+{
+    int count = 0;
+    int rc = run_topk(z, 1, K, k, idx_out, &count);
+    return rc < 0 ? rc : count;
+}
+
+int fredec_topk_batched(const double* z, int64_t B, int64_t K, int32_t k, int64_t* idx_out)
+{
+    int count = 0;
+    return run_topk(z, B, K, k, idx_out, &count);
+}
+
+int fredec_set_stream(void* cuda_stream)
+{
+    g.stream = static_cast<cudaStream_t>(cuda_stream);
+    return FREDEC_OK;
+}
+
+int fredec_last_timing(double out[4])
+{
+    if (!out) return FREDEC_EINVAL;
+    for (int i = 0; i < 4; ++i) out[i] = g.timing[i];
+    return FREDEC_OK;
+}
+
+int fredec_last_launches(void) { return g.launches; }
+
+int fredec_fp64_peak(int64_t iters, double* tflops_out, double* ms_out)
+{
+    if (iters < 1024 || !tflops_out) return FREDEC_EINVAL;
+    int rc = ensure_ready();
+    if (rc) return rc;
+    CK(g.sink.reserve(64));
+    const int blocks = g.sm_count * 8;  // 2048 threads per SM
+    cudaStream_t st = g.stream;
+    CK(launch_dfma(1024, blocks, g.sink.as<double>(), st));  // warm-up
+    CK(cudaEventRecord(g.ev[0], st));
+    CK(launch_dfma(iters, blocks, g.sink.as<double>(), st));
+    CK(cudaEventRecord(g.ev[1], st));
+    CK(cudaStreamSynchronize(st));
+    const double ms = ev_ms(0, 1);
+    *tflops_out = ms > 0.0 ? dfma_flops(iters, blocks) / (ms * 1e-3) * 1e-12 : 0.0;
+    if (ms_out) *ms_out = ms;
+    return FREDEC_OK;
+}
+
+int fredec_shutdown(void)
+{
+    DevBuf* bufs[] = {&g.in_t, &g.in_x, &g.in_w, &g.in_base, &g.in_z, &g.out_z, &g.out_idx, &g.out_chi2, &g.rec,
+                      &g.psi,  &g.xt,   &g.info, &g.ws,      &g.part_z, &g.part_i, &g.count, &g.sink};
+    for (DevBuf* b : bufs) b->release();
+    g.h_info.release();
+    g.h_count.release();
+    if (g.ready)
+        for (int i = 0; i < kNumEvents; ++i) cudaEventDestroy(g.ev[i]);
+    g.ready = false;
+    (void)cudaGetLastError();
+    return FREDEC_OK;
+}
+
+const char* fredec_strerror(int code)
+{
+    switch (code) {
+        case FREDEC_OK: return "ok";
+        case FREDEC_EINVAL: return "invalid argument";
+        case FREDEC_EDATA: return "invalid data (non-finite value, negative weight or zero total weight)";
+        case FREDEC_ESINGULAR: return "base functions are linearly dependent";
+        case FREDEC_ECUDA: return "CUDA error (see fredec_last_cuda_error)";
+        default: return code > 0 ? "ok (count)" : "unknown error";
+    }
+}
+
+int fredec_last_cuda_error(void) { return g.last_cuda; }
+
+int fredec_version(void) { return 100; }
+
+}  // extern "C"

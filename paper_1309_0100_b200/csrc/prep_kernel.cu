@@ -1,0 +1,174 @@
+// prep_kernel.cu -- steps a1-a3 of the scan: validate, centre, orthogonalise the base
+// model, pack per-observation records.  Once per scan, one CTA per series.
+//
+// Generalises the normalisations of PAPER.md:193-197 (eq. 18: <1> = 1, <x> = 0, ...) to an
+// arbitrary linear base model: the base functions are replaced by functions psi_j that are
+// orthonormal under <.>, and x by its residual after the base fit.  Then the (d+2)x(d+2)
+// system of PAPER.md:165-175 (eqs. 15, 16; Cholesky solve) has an identity leading block and
+// collapses to the 2x2 Schur complement the scan kernel solves per frequency.
+//
+// Orthogonalisation is modified Gram-Schmidt applied twice ("twice is enough"), in the
+// weighted inner product <u v> = sum_i w_i u_i v_i, with deterministic (fixed-order)
+// block reductions.
+#include "prep_kernel.cuh"
+
+namespace fredec {
+
+namespace {
+
+constexpr int kPrepThreads = 256;
+
+// Fixed-order block sum, result broadcast to all threads.  `red` = 32 doubles of smem.
+__device__ double block_sum(double v, double* red)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    __syncthreads();  // protect `red` from the previous call's readers
+    if (lane == 0) red[wid] = v;
+    __syncthreads();
+    double r = (lane < (kPrepThreads >> 5)) ? red[lane] : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) r += __shfl_xor_sync(0xffffffffu, r, o);
+    return r;
+}
+
+__device__ double block_min(double v, double* red)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    __syncthreads();
+    if (lane == 0) red[wid] = v;
+    __syncthreads();
+    double r = (lane < (kPrepThreads >> 5)) ? red[lane] : v;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) r = fmin(r, __shfl_xor_sync(0xffffffffu, r, o));
+    return r;
+}
+
+// <u v> over the series (u may alias v).
+__device__ double wdot(const double* __restrict__ w, const double* u, const double* v, int64_t N, double* red)
+{
+    double acc = 0.0;
+    for (int64_t i = threadIdx.x; i < N; i += kPrepThreads) acc = fma(w[i] * u[i], v[i], acc);
+    return block_sum(acc, red);
+}
+
+__global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p)
+{
+    __shared__ double red[32];
+    const int64_t b = blockIdx.x, N = p.N;
+    const int d = p.d;
+    const double* t = p.t + b * N;
+    const double* x = p.x + b * N;
+    const double* w = p.w + b * N;
+    const double* base = p.base ? p.base + b * (int64_t)d * N : nullptr;
+    double* psi = p.psi + b * (int64_t)d * N;  // [d][N]
+    double* xt = p.xt + b * N;                 // [N]
+    SeriesInfo* info = p.info + b;
+
+    // ---- a1: validate, W = <1>, time origin --------------------------------------------
+    double bad = 0.0, neg = 0.0, wsum = 0.0, tmin = INFINITY, tmax = -INFINITY;
+    for (int64_t i = threadIdx.x; i < N; i += kPrepThreads) {
+        double ti = t[i], xi = x[i], wi = w[i];
+        if (!isfinite(ti) || !isfinite(xi) || !isfinite(wi)) bad = 1.0;
+        if (wi < 0.0) neg = 1.0;
+        wsum += wi;
+        tmin = fmin(tmin, ti);
+        tmax = fmax(tmax, ti);
+        for (int j = 0; j < d; ++j)
+            if (!isfinite(base[(int64_t)j * N + i])) bad = 1.0;
+    }
+    bad = block_sum(bad + neg, red);
+    const double W = block_sum(wsum, red);
+    tmin = block_min(tmin, red);
+    tmax = -block_min(-tmax, red);
+    int status = 0;
+    if (bad != 0.0 || !(W > 0.0) || !isfinite(W)) status = -2;  // FREDEC_EDATA
+    const double t_mid = 0.5 * (tmin + tmax);
+
+    // ---- a2: orthonormal base psi (MGS, two sweeps) and residual x~ -----------------------
+    if (status == 0) {
+        for (int j = 0; j < d; ++j) {
+            double* v = psi + (int64_t)j * N;
+            for (int64_t i = threadIdx.x; i < N; i += kPrepThreads) v[i] = base[(int64_t)j * N + i];
+            __syncthreads();
+            const double n0 = wdot(w, v, v, N, red);
+            for (int sweep = 0; sweep < 2; ++sweep)
+                for (int k = 0; k < j; ++k) {
+                    const double* q = psi + (int64_t)k * N;
+                    const double r = wdot(w, q, v, N, red);
+                    for (int64_t i = threadIdx.x; i < N; i += kPrepThreads) v[i] = fma(-r, q[i], v[i]);
+                    __syncthreads();
+                }
+            const double n1 = wdot(w, v, v, N, red);
+            if (!(n1 > kTauBase * n0)) {
+                status = -3;  // FREDEC_ESINGULAR (uniform across the block)
+                break;
+            }
+            const double inv = 1.0 / sqrt(n1);
+            for (int64_t i = threadIdx.x; i < N; i += kPrepThreads) v[i] *= inv;
+            __syncthreads();
+        }
+    }
+    double chi2 = 0.0;
+    if (status == 0) {
+        for (int64_t i = threadIdx.x; i < N; i += kPrepThreads) xt[i] = x[i];
+        __syncthreads();
+        for (int sweep = 0; sweep < 2; ++sweep)
+            for (int k = 0; k < d; ++k) {
+                const double* q = psi + (int64_t)k * N;
+                const double r = wdot(w, q, xt, N, red);
+                for (int64_t i = threadIdx.x; i < N; i += kPrepThreads) xt[i] = fma(-r, q[i], xt[i]);
+                __syncthreads();
+            }
+        chi2 = wdot(w, xt, xt, N, red);
+    }
+    if (threadIdx.x == 0) {
+        info->W = W;
+        info->chi2_base = chi2;
+        info->t_mid = t_mid;
+        info->status = status;
+        info->pad = 0;
+    }
+    if (status != 0 || p.rec == nullptr) return;
+
+    // ---- a3: step constants and packing ---------------------------------------------------
+    const int RS = rec_stride(p.NB);
+    const int NBP = RS - kHdr;
+    const double dfR = p.df * (double)p.R;  // exact: R is a power of two
+    for (int pass = 0; pass < p.n_pass; ++pass) {
+        double* rec = p.rec + ((b * p.n_pass + pass) * N) * RS;
+        for (int64_t i = threadIdx.x; i < N; i += kPrepThreads) {
+            double* r = rec + i * RS;
+            const double tc = t[i] - t_mid;
+            double c1, s1, cR, sR;
+            sincospi(2.0 * frac_prod(p.df, tc), &s1, &c1);
+            sincospi(2.0 * frac_prod(dfR, tc), &sR, &cR);
+            const double wi = w[i];
+            r[0] = tc;
+            r[1] = 0.0;
+            r[2] = c1;
+            r[3] = s1;
+            r[4] = cR;
+            r[5] = sR;
+            r[6] = pass == 0 ? wi : 0.0;
+            r[7] = pass == 0 ? wi * xt[i] : 0.0;
+            for (int m = 0; m < NBP; ++m) {
+                const int j = pass * p.NB + m;
+                r[kHdr + m] = (m < p.NB && j < d) ? wi * psi[(int64_t)j * N + i] : 0.0;
+            }
+        }
+    }
+}
+
+}  // namespace
+
+cudaError_t launch_prep(const PrepParams& p, int64_t B, cudaStream_t stream)
+{
+    prep_kernel<<<(unsigned)B, kPrepThreads, 0, stream>>>(p);
+    return cudaGetLastError();
+}
+
+}  // namespace fredec

@@ -1,0 +1,26 @@
+// prep_kernel.cuh -- launch interface of the orthogonalisation / packing kernel.
+#pragma once
+#include "common.cuh"
+
+namespace fredec {
+
+struct PrepParams {
+    const double* t;     // [B][N]
+    const double* x;     // [B][N]
+    const double* w;     // [B][N]
+    const double* base;  // [B][d][N] or nullptr when d == 0
+    double* psi;         // workspace [B][d][N]
+    double* xt;          // workspace [B][N]
+    double* rec;         // out [B][n_pass][N][rec_stride(NB)], or nullptr: scalars only
+    SeriesInfo* info;    // out [B]
+    int64_t N;
+    int d;
+    int NB;      // base functions per pass
+    int n_pass;  // ceil(d / NB), >= 1
+    int R;       // grid steps per run (power of two)
+    double df;
+};
+
+cudaError_t launch_prep(const PrepParams& p, int64_t B, cudaStream_t stream);
+
+}  // namespace fredec

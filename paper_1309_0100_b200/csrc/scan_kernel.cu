@@ -1,0 +1,276 @@
+// scan_kernel.cu -- steps a4-a10: the periodogram scan kernel for sm_100a.
+//
+// For every grid frequency f_k the kernel forms the weighted trigonometric sums of
+// PAPER.md:165-171 (eqs. 15, 16) against the orthonormalised base (prep kernel):
+//
+//   YC = <x~ cos>, YS = <x~ sin>, CC = <cos^2>, CS = <cos sin>, (SS = <1> - CC)
+//   A_j = <psi_j cos>, B_j = <psi_j sin>,  j < NB
+//
+// and solves the 2x2 Schur complement (the last two steps of the Cholesky forward
+// substitution of PAPER.md:175/183) in the epilogue: z = a_d^2 + a_{d+1}^2.
+//
+// Work decomposition: a thread owns a RUN of R consecutive grid frequencies and keeps their
+// R*(4+2NB) sums in registers.  Observation records are staged tile by tile into shared
+// memory with 1-D TMA bulk copies (cp.async.bulk + mbarrier, double buffered) and read as
+// warp-broadcast LDS.128.  For each observation the thread seeds (cos, sin) at its first
+// frequency from an exactly range-reduced phase and then advances along the frequency axis
+// with the rotation recurrence (cos, sin) <- (cos, sin) x (cos d_i, sin d_i).
+// No per-pair sincos.  Partial sums of warps that split the observations of a tile are
+// combined in a fixed order through shared memory (bitwise reproducible).
+#include "scan_kernel.cuh"
+
+namespace fredec {
+
+namespace {
+
+constexpr int kMaxScanThreads = 256;
+
+template <int R, int NB>
+struct Acc {
+    double YC[R], YS[R], CC[R], CS[R];
+    double A[R][NB > 0 ? NB : 1], B[R][NB > 0 ? NB : 1];
+
+    __device__ __forceinline__ void clear()
+    {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            YC[r] = YS[r] = CC[r] = CS[r] = 0.0;
+#pragma unroll
+            for (int j = 0; j < NB; ++j) A[r][j] = B[r][j] = 0.0;
+        }
+    }
+    // visit every accumulator with a compile-time index (used by the split reduction)
+    template <class F>
+    __device__ __forceinline__ void for_each(F&& f)
+    {
+        int a = 0;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            f(YC[r], a++);
+            f(YS[r], a++);
+            f(CC[r], a++);
+            f(CS[r], a++);
+#pragma unroll
+            for (int j = 0; j < NB; ++j) {
+                f(A[r][j], a++);
+                f(B[r][j], a++);
+            }
+        }
+    }
+};
+
+template <int R, int NB>
+__global__ void __launch_bounds__(kMaxScanThreads, 1) scan_kernel(ScanParams p)
+{
+    constexpr int RS = rec_stride(NB);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    __shared__ __align__(8) uint64_t bar[2];
+    double* const tile_buf = reinterpret_cast<double*>(smem_raw);
+
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int FW = p.FW, S = p.S, TI = p.TI;
+    const int fw = wid % FW, sp = wid / FW;
+    const int64_t b = blockIdx.y;
+    const SeriesInfo info = p.info[b];
+    if (info.status != 0) return;  // uniform over the CTA; the host reports the error
+
+    const int64_t N = p.N, K = p.K;
+    const int64_t run = (int64_t)blockIdx.x * (FW * 32) + fw * 32 + lane;
+    const int64_t k0 = run * R;
+    const bool active = k0 < K;
+    const double fk0 = fma((double)k0, p.df, p.f0);  // S1: the run starts on fl(f0 + k0 df)
+    const double* rec = p.rec + ((b * p.n_pass + p.pass) * N) * RS;
+
+    const int ntiles = (int)((N + TI - 1) / TI);
+    if (tid == 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    auto issue = [&](int tile) {
+        const int64_t first = (int64_t)tile * TI;
+        const int rows = (int)min((int64_t)TI, N - first);
+        const uint32_t bytes = (uint32_t)rows * RS * 8u;
+        uint64_t* mb = &bar[tile & 1];
+        mbar_expect_tx(mb, bytes);
+        bulk_g2s(tile_buf + (size_t)(tile & 1) * TI * RS, rec + first * RS, bytes, mb);
+    };
+    if (tid == 0) issue(0);
+
+    Acc<R, NB> acc;
+    acc.clear();
+
+    const int rows_per_split = TI / S;
+    for (int tile = 0; tile < ntiles; ++tile) {
+        if (tid == 0 && tile + 1 < ntiles) issue(tile + 1);  // stage (tile+1)&1 was released by the
+                                                             // __syncthreads that ended tile-1
+        mbar_wait(&bar[tile & 1], (uint32_t)((tile >> 1) & 1));
+        const int rows = (int)min((int64_t)TI, N - (int64_t)tile * TI);
+        const int i_begin = sp * rows_per_split;
+        const int i_end = min(rows, i_begin + rows_per_split);
+        const double* tb = tile_buf + (size_t)(tile & 1) * TI * RS;
+        if (active) {
+            for (int i = i_begin; i < i_end; ++i) {
+                const double2* r2 = reinterpret_cast<const double2*>(tb + (size_t)i * RS);
+                const double2 h0 = r2[0];  // t', -
+                const double2 h1 = r2[1];  // cos d, sin d
+                const double2 h3 = r2[3];  // w, y
+                double pj[NB > 0 ? NB : 1];
+#pragma unroll
+                for (int j = 0; j < NB; j += 2) {
+                    const double2 q = r2[kHdr / 2 + j / 2];
+                    pj[j] = q.x;
+                    if (j + 1 < NB) pj[j + 1] = q.y;
+                }
+                // a5: seed at the run's first frequency from the exactly reduced phase
+                double c, s;
+                sincospi(2.0 * frac_prod(fk0, h0.x), &s, &c);
+                const double cd = h1.x, sd = h1.y, w = h3.x, y = h3.y;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    // a6: accumulate
+                    acc.YC[r] = fma(y, c, acc.YC[r]);
+                    acc.YS[r] = fma(y, s, acc.YS[r]);
+                    const double u = w * c;
+                    acc.CC[r] = fma(u, c, acc.CC[r]);
+                    acc.CS[r] = fma(u, s, acc.CS[r]);
+#pragma unroll
+                    for (int j = 0; j < NB; ++j) {
+                        acc.A[r][j] = fma(pj[j], c, acc.A[r][j]);
+                        acc.B[r][j] = fma(pj[j], s, acc.B[r][j]);
+                    }
+                    // a7: rotate to the next grid frequency
+                    if (r + 1 < R) {
+                        const double cn = fma(c, cd, -(s * sd));
+                        const double sn = fma(s, cd, c * sd);
+                        c = cn;
+                        s = sn;
+                    }
+                }
+            }
+        }
+        __syncthreads();
+    }
+
+    // ---- a8: combine the observation split in a fixed order ------------------------------
+    if (S > 1) {
+        double* red = tile_buf;  // every bulk copy has completed and been consumed
+        const int nthr_f = FW * 32, col = fw * 32 + lane;
+        for (int q = 1; q < S; ++q) {
+            if (sp == q) acc.for_each([&](double& v, int a) { red[a * nthr_f + col] = v; });
+            __syncthreads();
+            if (sp == 0) acc.for_each([&](double& v, int a) { v += red[a * nthr_f + col]; });
+            __syncthreads();
+        }
+    }
+    if (sp != 0 || !active) return;
+
+    // ---- a9: per-frequency solve ------------------------------------------------------------
+    double* zp = p.z + b * K + k0;
+    double zr[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        double Saa = 0.0, Sab = 0.0, Sbb = 0.0;
+#pragma unroll
+        for (int j = 0; j < NB; ++j) {
+            Saa = fma(acc.A[r][j], acc.A[r][j], Saa);
+            Sab = fma(acc.A[r][j], acc.B[r][j], Sab);
+            Sbb = fma(acc.B[r][j], acc.B[r][j], Sbb);
+        }
+        double YC = acc.YC[r], YS = acc.YS[r], CC = acc.CC[r], CS = acc.CS[r];
+        if (p.n_pass > 1) {  // multi-pass: carry the seven partial sums through global memory
+            double* wsp = p.ws + (b * 7) * p.Kpad + k0 + r;
+            if (p.pass > 0) {
+                YC += wsp[0 * p.Kpad];
+                YS += wsp[1 * p.Kpad];
+                CC += wsp[2 * p.Kpad];
+                CS += wsp[3 * p.Kpad];
+                Saa += wsp[4 * p.Kpad];
+                Sab += wsp[5 * p.Kpad];
+                Sbb += wsp[6 * p.Kpad];
+            }
+            if (p.pass + 1 < p.n_pass) {
+                wsp[0 * p.Kpad] = YC;
+                wsp[1 * p.Kpad] = YS;
+                wsp[2 * p.Kpad] = CC;
+                wsp[3 * p.Kpad] = CS;
+                wsp[4 * p.Kpad] = Saa;
+                wsp[5 * p.Kpad] = Sab;
+                wsp[6 * p.Kpad] = Sbb;
+            }
+        }
+        const double SS = info.W - CC;  // <sin^2> = <1> - <cos^2>
+        const double Scc = CC - Saa, Scs = CS - Sab, Sss = SS - Sbb;
+        double z = 0.0, ys = YS, piv2 = Sss;
+        if (Scc > kTauTrial * CC) {  // S6: otherwise the cos column is in the span of the base
+            const double q = Scs / Scc;
+            z = YC * YC / Scc;
+            ys = fma(-q, YC, YS);
+            piv2 = fma(-q, Scs, Sss);
+        }
+        if (piv2 > kTauTrial * SS) z = fma(ys, ys / piv2, z);
+        zr[r] = z;
+    }
+    if (p.pass + 1 < p.n_pass) return;
+
+    // ---- a10: store -----------------------------------------------------------------------
+    if (k0 + R <= K && (reinterpret_cast<uintptr_t>(zp) & 15) == 0 && R % 2 == 0) {
+#pragma unroll
+        for (int r = 0; r < R; r += 2) reinterpret_cast<double2*>(zp)[r / 2] = make_double2(zr[r], zr[r + 1]);
+    } else {
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            if (k0 + r < K) zp[r] = zr[r];
+    }
+}
+
+template <int R, int NB>
+cudaError_t launch_one(const ScanParams& p, int64_t B, cudaStream_t stream)
+{
+    const size_t smem = scan_smem_bytes(R, NB, p);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(scan_kernel<R, NB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             200 * 1024);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const int64_t runs = (p.K + R - 1) / R;
+    const int64_t per_cta = (int64_t)p.FW * 32;
+    dim3 grid((unsigned)((runs + per_cta - 1) / per_cta), (unsigned)B);
+    scan_kernel<R, NB><<<grid, p.FW * p.S * 32, smem, stream>>>(p);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+size_t scan_smem_bytes(int R, int NB, const ScanParams& p)
+{
+    const size_t tiles = 2 * (size_t)p.TI * rec_stride(NB) * 8;
+    const size_t red = p.S > 1 ? (size_t)R * (4 + 2 * NB) * p.FW * 32 * 8 : 0;
+    return tiles > red ? tiles : red;
+}
+
+#define FREDEC_SCAN_CONFIGS(X) \
+    X(8, 0) X(8, 1) X(8, 2) X(8, 3) X(4, 4) X(4, 5) X(4, 6) X(4, 7) X(4, 8) X(4, 9)
+
+bool scan_config_supported(int R, int NB)
+{
+#define X(r, nb) \
+    if (R == r && NB == nb) return true;
+    FREDEC_SCAN_CONFIGS(X)
+#undef X
+    return false;
+}
+
+cudaError_t launch_scan(int R, int NB, const ScanParams& p, int64_t B, cudaStream_t stream)
+{
+#define X(r, nb) \
+    if (R == r && NB == nb) return launch_one<r, nb>(p, B, stream);
+    FREDEC_SCAN_CONFIGS(X)
+#undef X
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace fredec

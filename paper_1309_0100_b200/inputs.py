@@ -197,6 +197,25 @@ def random_series(seed: int, N: int, d: int, t_span: float = 100.0, noise: float
     sigma = rng.uniform(0.5, 2.0, N)
     x = (2.0 * np.cos(TWO_PI * t * (7.3 / t_span) + 0.3) + 0.7 * np.sin(TWO_PI * t * (19.1 / t_span))
          + 0.05 * t / t_span + rng.normal(0.0, noise, N) * sigma)
+    return t, x, 1.0 / sigma**2, mixed_base(t, d, t_span)
+
+
+def mixed_base(t: np.ndarray, d: int, t_span: float) -> np.ndarray:
+    """A well-conditioned base model of d functions: 1, t, then cos/sin pairs at fixed
+    frequencies (2.3137 + 1.7291 m)/t_span (accepted sinusoids), t^2 when d is even
+    and > 2; plain polynomials for d <= 3.  Returns [d, N]."""
+    N = t.shape[0]
+    if d == 0:
+        return np.zeros((0, N))
     tc = (t - t.mean()) / t_span
-    base = np.stack([tc**j for j in range(d)]) if d > 0 else np.zeros((0, N))
-    return t, x, 1.0 / sigma**2, base
+    if d <= 3:
+        return np.stack([tc**j for j in range(d)])
+    rows = [np.ones_like(tc), tc]
+    m = 0
+    while len(rows) + 2 <= d:
+        nu = 2.3137 + 1.7291 * m
+        rows += [np.cos(TWO_PI * nu * tc), np.sin(TWO_PI * nu * tc)]
+        m += 1
+    if len(rows) < d:
+        rows.append(tc**2)
+    return np.stack(rows)

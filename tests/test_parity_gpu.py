@@ -1,0 +1,265 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerance from BASELINE.json:north_star:
+|dz| <= 1e-9 * max(z); top-k indices identical."""
+import numpy as np
+import pytest
+
+from paper_1309_0100_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+RTOL_MAXZ = 1e-9
+
+
+@pytest.fixture(scope="module")
+def fr():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1309_0100_b200 import build
+    build.build()
+    import paper_1309_0100_b200 as fr
+    fr.lib()
+    return fr
+
+
+def _dev(*arrays):
+    import torch
+    return [None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in arrays]
+
+
+def gpu_scan(fr, t, x, w, base, f0, df, K, device=True):
+    if device:
+        dt, dx, dw, db = _dev(t, x, w, base if base is not None and base.shape[0] else None)
+        z = fr.fredec_scan(dt, dx, dw, db, f0, df, K)
+        return z.cpu().numpy()
+    return fr.fredec_scan(t, x, w, base, f0, df, K)
+
+
+def assert_parity(z_gpu, z_ref, what=""):
+    zmax = float(np.max(z_ref))
+    err = float(np.max(np.abs(z_gpu - z_ref)))
+    assert np.all(np.isfinite(z_gpu)), what
+    assert err <= RTOL_MAXZ * zmax, f"{what}: max|dz| = {err:.3e} > 1e-9 * {zmax:.3e}"
+    return err / zmax
+
+
+# ------------------------------------------------------------------ configs 1-3 in full
+@pytest.mark.parametrize("cfg", [1, 2, 3])
+def test_config_full_parity_and_topk(fr, oracle_mod, cfg):
+    wl = inputs.config(cfg)
+    t, x, w, base = wl.series(0)
+    z_ref = oracle_mod.scan(t, x, w, base, wl.f0, wl.df, wl.K, threads=0)
+    z = gpu_scan(fr, t, x, w, base, wl.f0, wl.df, wl.K)
+    assert_parity(z, z_ref, wl.name)
+    chi2 = fr.fredec_chi2_base(t, x, w, base)
+    chi2_ref = oracle_mod.chi2_base(t, x, w, base)
+    assert abs(chi2 - chi2_ref) <= 1e-12 * chi2_ref
+    assert z.min() >= 0.0 and z.max() <= chi2 * (1 + 1e-12)
+    # peaks: GPU top-k on GPU z == oracle top-k on oracle z (end to end), and bit-exact on the same z
+    idx_ref, cnt_ref = oracle_mod.topk(z_ref, wl.topk)
+    idx, cnt = fr.fredec_topk(z, wl.topk)
+    assert cnt == cnt_ref and idx.tolist() == idx_ref.tolist()
+    idx_same, cnt_same = oracle_mod.topk(z, wl.topk)
+    assert idx.tolist() == idx_same.tolist()
+
+
+# ------------------------------------------------------------------ config 4, bench launch configuration
+def test_config4_full_size_sampled(fr, oracle_mod):
+    """Full N = 10 000 x K = 2 000 000 scan exactly as bench.py launches it; the oracle
+    evaluates a sample of grid points one by one (each is an independent fit)."""
+    import torch
+    from test_oracle_pins import grid_frequencies
+    wl = inputs.config(4)
+    t, x, w, base = wl.series(0)
+    dt, dx, dw, db = _dev(t, x, w, base)
+    z = fr.fredec_scan(dt, dx, dw, db, wl.f0, wl.df, wl.K)
+    idx_gpu, cnt = fr.fredec_topk(z, wl.topk)
+    z = z.cpu().numpy()
+    idx_gpu = idx_gpu.cpu().numpy()
+    rng = np.random.Generator(np.random.PCG64(44))
+    ks = np.unique(np.concatenate([
+        rng.integers(0, wl.K, 600), np.arange(0, 40), np.arange(wl.K - 40, wl.K),
+        idx_gpu[idx_gpu >= 0], np.arange(1_000_000 - 20, 1_000_000 + 20)]))
+    from fractions import Fraction
+    zmax = float(z.max())
+    worst = 0.0
+    for k in ks:
+        fk = float(Fraction(int(k)) * Fraction(wl.df) + Fraction(wl.f0))   # S1 grid frequency
+        zr = oracle_mod.scan(t, x, w, base, fk, 1.0, 1)[0]
+        worst = max(worst, abs(zr - z[k]))
+    assert worst <= RTOL_MAXZ * zmax, f"max|dz| = {worst:.3e} vs max z {zmax:.3e}"
+    chi2 = oracle_mod.chi2_base(t, x, w, base)
+    assert z.min() >= 0.0 and zmax <= chi2 * (1 + 1e-12)
+    # top-k on the full array: bit-exact against the oracle's peak finder on the same z
+    idx_ref, cnt_ref = oracle_mod.topk(z, wl.topk)
+    assert cnt == cnt_ref and idx_gpu.tolist() == idx_ref.tolist()
+    # a contiguous slice in full (several tiles of frequencies, includes a ragged start)
+    k1, n = 777_771, 3000
+    f1 = float(Fraction(k1) * Fraction(wl.df) + Fraction(wl.f0))
+    z_slice = oracle_mod.scan(t, x, w, base, f1, wl.df, n, threads=0)
+    assert np.max(np.abs(z_slice - z[k1:k1 + n])) <= RTOL_MAXZ * zmax
+
+
+# ------------------------------------------------------------------ config 5 (batched)
+def test_config5_reduced_batch_full_parity(fr, oracle_mod):
+    wl = inputs.config(5, B=12, K=20_000)
+    z_ref = oracle_mod.scan_batched(wl.t, wl.x, wl.w, wl.base_funcs, wl.f0, wl.df, wl.K, threads=0)
+    dt, dx, dw, db = _dev(wl.t, wl.x, wl.w, wl.base_funcs)
+    z = fr.fredec_scan_batched(dt, dx, dw, db, wl.f0, wl.df, wl.K)
+    idx = fr.fredec_topk_batched(z, wl.topk).cpu().numpy()
+    z = z.cpu().numpy()
+    for b in range(wl.B):
+        assert_parity(z[b], z_ref[b], f"series {b}")
+        assert idx[b].tolist() == oracle_mod.topk(z_ref[b], wl.topk)[0].tolist()
+    chi2 = fr.fredec_chi2_base_batched(wl.t, wl.x, wl.w, wl.base_funcs)
+    for b in range(wl.B):
+        assert abs(chi2[b] - oracle_mod.chi2_base(*wl.series(b))) <= 1e-12 * chi2[b]
+
+
+@pytest.mark.slow
+def test_config5_full_size_sampled(fr, oracle_mod):
+    """B = 4096 x N = 500 x K = 100 000 as bench.py launches it (3.3 GB of z): sampled
+    (series, frequency) points against the oracle, and top-5 of sampled series bit-exact."""
+    import torch
+    from fractions import Fraction
+    wl = inputs.config(5)
+    dt, dx, dw, db = _dev(wl.t, wl.x, wl.w, wl.base_funcs)
+    z = fr.fredec_scan_batched(dt, dx, dw, db, wl.f0, wl.df, wl.K)
+    idx = fr.fredec_topk_batched(z, wl.topk).cpu().numpy()
+    rng = np.random.Generator(np.random.PCG64(55))
+    for b in np.unique(np.concatenate([[0, wl.B - 1], rng.integers(0, wl.B, 14)])):
+        zb = z[b].cpu().numpy()
+        t, x, w, base = wl.series(int(b))
+        zmax = float(zb.max())
+        ks = np.unique(np.concatenate([rng.integers(0, wl.K, 40), [0, wl.K - 1], idx[b][idx[b] >= 0]]))
+        for k in ks:
+            fk = float(Fraction(int(k)) * Fraction(wl.df) + Fraction(wl.f0))
+            zr = oracle_mod.scan(t, x, w, base, fk, 1.0, 1)[0]
+            assert abs(zr - zb[k]) <= RTOL_MAXZ * zmax
+        assert idx[b].tolist() == oracle_mod.topk(zb, wl.topk)[0].tolist()
+
+
+# ------------------------------------------------------------------ shapes, tails, passes
+@pytest.mark.parametrize("d", [0, 1, 2, 3, 4, 5, 7, 9, 10, 13, 20])
+def test_base_sizes_and_multipass(fr, oracle_mod, d):
+    t, x, w, base = inputs.random_series(300 + d, 333, d)
+    f0, df, K = 0.004, 0.0007, 1237          # K not a multiple of any run length
+    z_ref = oracle_mod.scan(t, x, w, base, f0, df, K, threads=0)
+    z = gpu_scan(fr, t, x, w, base, f0, df, K)
+    assert_parity(z, z_ref, f"d={d}")
+
+
+@pytest.mark.parametrize("N,K", [(4, 1), (5, 7), (31, 8), (129, 33), (257, 4097), (1000, 100_003)])
+def test_ragged_sizes(fr, oracle_mod, N, K):
+    t, x, w, base = inputs.random_series(N + K, N, 1)
+    f0, df = 0.01, 0.9 / K
+    z_ref = oracle_mod.scan(t, x, w, base, f0, df, K, threads=0)
+    z = gpu_scan(fr, t, x, w, base, f0, df, K)
+    assert_parity(z, z_ref, f"N={N},K={K}")
+
+
+def test_host_and_device_pointers_agree_bitwise(fr):
+    wl = inputs.config(2, K=5000)
+    t, x, w, base = wl.series(0)
+    za = gpu_scan(fr, t, x, w, base, wl.f0, wl.df, wl.K, device=True)
+    zb = gpu_scan(fr, t, x, w, base, wl.f0, wl.df, wl.K, device=False)
+    zc = gpu_scan(fr, t, x, w, base, wl.f0, wl.df, wl.K, device=True)
+    assert np.array_equal(za, zb) and np.array_equal(za, zc)      # also: run-to-run reproducible
+
+
+def test_large_phase_accuracy(fr, oracle_mod):
+    """t ~ 2.4e6 (Julian-date like), f up to 20: phases of ~5e7 turns."""
+    t, x, w, _ = inputs.random_series(77, 400, 0, t_span=300.0)
+    t = t + 2.45e6
+    base = inputs.base_offset_trend(t - 2.45e6)
+    f0, df, K = 10.0, 0.001, 10_000
+    z_ref = oracle_mod.scan(t, x, w, base, f0, df, K, threads=0)
+    z = gpu_scan(fr, t, x, w, base, f0, df, K)
+    assert_parity(z, z_ref, "large phase")
+
+
+def test_unsorted_times_zero_weights(fr, oracle_mod):
+    t, x, w, _ = inputs.random_series(5, 200, 0)
+    perm = np.random.Generator(np.random.PCG64(1)).permutation(200)
+    t, x, w = t[perm], x[perm], w[perm].copy()
+    w[::7] = 0.0
+    base = inputs.base_offset(t)
+    z_ref = oracle_mod.scan(t, x, w, base, 0.01, 0.001, 2000)
+    z = gpu_scan(fr, t, x, w, base, 0.01, 0.001, 2000)
+    assert_parity(z, z_ref)
+
+
+def test_singular_trial_frequency(fr, oracle_mod):
+    """S6: f = 0 with a constant in the base, and f equal to a base frequency: z = 0."""
+    t, x, w, _ = inputs.random_series(6, 80, 0)
+    z = gpu_scan(fr, t, x, w, inputs.base_offset(t), 0.0, 0.01, 5)
+    z_ref = oracle_mod.scan(t, x, w, inputs.base_offset(t), 0.0, 0.01, 5)
+    assert z[0] == 0.0 and np.all(np.isfinite(z))
+    assert np.max(np.abs(z - z_ref)) <= RTOL_MAXZ * z_ref.max()
+    base = inputs.base_offset_sinusoids(t, [8.0])
+    z = gpu_scan(fr, t, x, w, base, 1.0 / 8.0, 1.0, 1)
+    assert z[0] == 0.0
+    z = gpu_scan(fr, t, x, w, None, 0.0, 0.01, 2)              # d = 0, f = 0
+    assert abs(z[0] - np.sum(w * x) ** 2 / np.sum(w)) <= 1e-12 * np.sum(w * x * x)
+
+
+def test_error_codes(fr):
+    import paper_1309_0100_b200 as m
+    t, x, w, base = inputs.random_series(9, 50, 1)
+
+    def code(fn):
+        with pytest.raises(m.FredecError) as e:
+            fn()
+        return e.value.code
+
+    bad = x.copy(); bad[3] = np.nan
+    assert code(lambda: fr.fredec_scan(t, bad, w, base, 0.01, 0.01, 10)) == m.FREDEC_EDATA
+    neg = w.copy(); neg[0] = -1.0
+    assert code(lambda: fr.fredec_scan(t, x, neg, base, 0.01, 0.01, 10)) == m.FREDEC_EDATA
+    assert code(lambda: fr.fredec_scan(t, x, 0 * w, base, 0.01, 0.01, 10)) == m.FREDEC_EDATA
+    dep = np.stack([np.ones_like(t), 3 * np.ones_like(t)])
+    assert code(lambda: fr.fredec_scan(t, x, w, dep, 0.01, 0.01, 10)) == m.FREDEC_ESINGULAR
+    assert code(lambda: fr.fredec_scan(t, x, w, base, 0.01, 0.0, 10)) == m.FREDEC_EINVAL
+    assert code(lambda: fr.fredec_scan(t, x, w, base, -0.1, 0.01, 10)) == m.FREDEC_EINVAL
+    assert code(lambda: fr.fredec_scan(t[:3], x[:3], w[:3], base[:, :3], 0.1, 0.01, 10)) == m.FREDEC_EINVAL
+    assert code(lambda: fr.fredec_topk(np.zeros(5), 6)) == m.FREDEC_EINVAL
+    # the library still works after errors
+    z = fr.fredec_scan(t, x, w, base, 0.01, 0.01, 10)
+    assert np.all(np.isfinite(z))
+
+
+# ------------------------------------------------------------------ top-k, bit-exact
+@pytest.mark.parametrize("z,k", [
+    ([0, 1, 0, 3, 0, 2, 0], 3), ([0, 1, 0, 3, 0, 2, 0], 5), ([5, 1, 0, 1, 7], 2),
+    ([0, 2, 2, 2, 0, 2, 0], 4), ([1, 2, 3, 4, 5], 2), ([5, 4, 3, 2, 1], 2), ([3, 3, 3, 3], 2),
+    ([0, 4, 0, 4, 0, 4], 3), ([7], 1), ([0, float("nan"), 0, 1, 0], 2),
+])
+def test_topk_hand_cases(fr, oracle_mod, z, k):
+    z = np.array(z, dtype=np.float64)
+    idx, cnt = fr.fredec_topk(z, k)
+    idx_ref, cnt_ref = oracle_mod.topk(z, k)
+    assert cnt == cnt_ref and idx.tolist() == idx_ref.tolist()
+
+
+@pytest.mark.parametrize("K,k", [(1000, 1), (1000, 10), (4097, 32), (50_000, 33), (300_000, 100),
+                                 (1_000_003, 257), (2_000_000, 1024)])
+def test_topk_random_with_ties(fr, oracle_mod, K, k):
+    rng = np.random.Generator(np.random.PCG64(K + k))
+    z = np.round(rng.gamma(1.0, 5.0, K), 1)          # coarse values: many exact ties and plateaus
+    z[rng.integers(0, K, 20)] = z.max() + 1.0        # tied global maxima
+    idx, cnt = fr.fredec_topk(z, k)
+    idx_ref, cnt_ref = oracle_mod.topk(z, k)
+    assert cnt == cnt_ref and np.array_equal(idx, idx_ref)
+    import torch
+    idx_d, cnt_d = fr.fredec_topk(torch.from_numpy(z).cuda(), k)
+    assert cnt_d == cnt_ref and np.array_equal(idx_d.cpu().numpy(), idx_ref)
+
+
+def test_topk_batched_matches_single(fr, oracle_mod):
+    rng = np.random.Generator(np.random.PCG64(3))
+    z = rng.gamma(1.0, 5.0, (37, 10_001))
+    z[5, :] = 1.0                                     # a series with a single plateau peak
+    z[6, :] = np.arange(10_001)                       # monotone
+    idx = fr.fredec_topk_batched(z, 5)
+    for b in range(z.shape[0]):
+        assert idx[b].tolist() == oracle_mod.topk(z[b], 5)[0].tolist()
