@@ -107,6 +107,20 @@ int fredec_chi2_base_batched(const double* t, const double* x, const double* w, 
 int fredec_topk(const double* z, int64_t K, int32_t k, int64_t* idx_out);
 int fredec_topk_batched(const double* z, int64_t B, int64_t K, int32_t k, int64_t* idx_out);
 
+/*
+ * fredec_scan_topk -- the whole hot path in one call: fredec_scan followed by fredec_topk on
+ * the periodogram while it is still in device memory (one phase-1 iteration of PAPER.md:201).
+ * z_out may be NULL when only the peaks are wanted (the periodogram then stays in a
+ * library-owned device buffer and is not copied out).  Other arguments as above.
+ * Returns the number of peaks written (single series) / FREDEC_OK (batched), or an error.
+ */
+int fredec_scan_topk(const double* t, const double* x, const double* w, int64_t N,
+                     const double* base_funcs, int32_t d, double f0, double df, int64_t K,
+                     double* z_out, int32_t k, int64_t* idx_out);
+int fredec_scan_topk_batched(const double* t, const double* x, const double* w, int64_t B, int64_t N,
+                             const double* base_funcs, int32_t d, double f0, double df, int64_t K,
+                             double* z_out, int32_t k, int64_t* idx_out);
+
 /* ----------------------------------------------------------------- runtime control */
 
 /* Stream on which all work is enqueued (a cudaStream_t passed as void*); NULL = default. */

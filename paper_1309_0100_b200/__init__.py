@@ -7,6 +7,6 @@ from ._binding import (  # noqa: F401
     FREDEC_D_MAX, FREDEC_ECUDA, FREDEC_EDATA, FREDEC_EINVAL, FREDEC_ESINGULAR, FREDEC_OK,
     FREDEC_TOPK_MAX, FredecError, LIB_PATH,
     fredec_chi2_base, fredec_chi2_base_batched, fredec_fp64_peak, fredec_last_launches,
-    fredec_last_timing, fredec_scan, fredec_scan_batched, fredec_set_stream, fredec_shutdown,
+    fredec_last_timing, fredec_scan, fredec_scan_batched, fredec_scan_topk, fredec_scan_topk_batched, fredec_set_stream, fredec_shutdown,
     fredec_topk, fredec_topk_batched, fredec_version, lib,
 )

@@ -23,6 +23,8 @@ _P, _I64, _I32, _F64 = C.c_void_p, C.c_int64, C.c_int32, C.c_double
 SIGNATURES = {
     "fredec_scan": (C.c_int, [_P, _P, _P, _I64, _P, _I32, _F64, _F64, _I64, _P]),
     "fredec_scan_batched": (C.c_int, [_P, _P, _P, _I64, _I64, _P, _I32, _F64, _F64, _I64, _P]),
+    "fredec_scan_topk": (C.c_int, [_P, _P, _P, _I64, _P, _I32, _F64, _F64, _I64, _P, _I32, _P]),
+    "fredec_scan_topk_batched": (C.c_int, [_P, _P, _P, _I64, _I64, _P, _I32, _F64, _F64, _I64, _P, _I32, _P]),
     "fredec_chi2_base": (C.c_int, [_P, _P, _P, _I64, _P, _I32, _P]),
     "fredec_chi2_base_batched": (C.c_int, [_P, _P, _P, _I64, _I64, _P, _I32, _P]),
     "fredec_topk": (C.c_int, [_P, _I64, _I32, _P]),
@@ -127,6 +129,35 @@ def fredec_scan_batched(t, x, w, base_funcs, f0, df, K, z_out=None):
     _check(lib().fredec_scan_batched(pt, px, pw, B, N, pb, d, float(f0), float(df), int(K), pz),
            "fredec_scan_batched")
     return z
+
+
+def fredec_scan_topk(t, x, w, base_funcs, f0, df, K, k, z_out=None, idx_out=None, want_z=True):
+    """Scan + peaks in one call.  Returns (z or None, idx[k], count)."""
+    N = int(t.shape[-1])
+    d = 0 if base_funcs is None else int(base_funcs.shape[0])
+    if d == 0:
+        base_funcs = None
+    z = (_empty_like_kind(t, (int(K),)) if z_out is None else z_out) if want_z else None
+    idx = _empty_like_kind(t, (int(k),), np.int64) if idx_out is None else idx_out
+    (pt, kt), (px, kx), (pw, kw), (pb, kb), (pz, kz) = map(_ptr, (t, x, w, base_funcs, z))
+    pi, ki = _ptr(idx, np.int64)
+    count = _check(lib().fredec_scan_topk(pt, px, pw, N, pb, d, float(f0), float(df), int(K), pz,
+                                          int(k), pi), "fredec_scan_topk")
+    return z, idx, count
+
+
+def fredec_scan_topk_batched(t, x, w, base_funcs, f0, df, K, k, z_out=None, idx_out=None, want_z=True):
+    B, N = int(t.shape[0]), int(t.shape[1])
+    d = 0 if base_funcs is None else int(base_funcs.shape[1])
+    if d == 0:
+        base_funcs = None
+    z = (_empty_like_kind(t, (B, int(K))) if z_out is None else z_out) if want_z else None
+    idx = _empty_like_kind(t, (B, int(k)), np.int64) if idx_out is None else idx_out
+    (pt, kt), (px, kx), (pw, kw), (pb, kb), (pz, kz) = map(_ptr, (t, x, w, base_funcs, z))
+    pi, ki = _ptr(idx, np.int64)
+    _check(lib().fredec_scan_topk_batched(pt, px, pw, B, N, pb, d, float(f0), float(df), int(K), pz,
+                                          int(k), pi), "fredec_scan_topk_batched")
+    return z, idx
 
 
 def fredec_chi2_base(t, x, w, base_funcs) -> float:

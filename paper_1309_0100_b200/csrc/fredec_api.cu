@@ -65,7 +65,7 @@ struct HostBuf {
     }
 };
 
-constexpr int kNumEvents = 5;
+constexpr int kNumEvents = 7;
 
 struct State {
     bool ready = false;
@@ -202,27 +202,40 @@ float ev_ms(int a, int b)
     return ms;
 }
 
-// Shared body of scan / chi2_base: with_scan == false runs only the prep kernel.
-int run_series(const double* t, const double* x, const double* w, int64_t B, int64_t N,
-               const double* base_funcs, int32_t d, double f0, double df, int64_t K,
-               double* z_out, double* chi2_out, bool with_scan)
+// ---------------------------------------------------------------------------------------
+// A compute call is assembled from three enqueue steps on g.stream and one finish:
+//   begin_call -> [enqueue_series] -> [enqueue_topk] -> finish_call (copies out, one sync)
+// Events: 0 start | 1 prep | 2 scan | 3 (scan done) | 4 topk | 5 (topk done) | 6 end.
+// ---------------------------------------------------------------------------------------
+struct Call {
+    int64_t B = 0;
+    bool has_series = false, has_topk = false;
+    double* dz = nullptr;     // device periodogram [B][K]
+    double* hz = nullptr;     // host destination of z, if any
+    size_t z_count = 0;
+    int64_t* didx = nullptr;  // device peak indices [B][k]
+    int64_t* hidx = nullptr;
+    size_t idx_count = 0;
+};
+
+int begin_call()
 {
-    int rc = check_series_args(t, x, w, B, N, base_funcs, d);
-    if (rc) return rc;
-    if (with_scan) {
-        if (!z_out || K < 1 || !(df > 0.0) || !(f0 >= 0.0) || !std::isfinite(f0) || !std::isfinite(df))
-            return FREDEC_EINVAL;
-        if (!std::isfinite(f0 + df * (double)K)) return FREDEC_EINVAL;
-    } else if (!chi2_out) {
-        return FREDEC_EINVAL;
-    }
-    rc = ensure_ready();
+    int rc = ensure_ready();
     if (rc) return rc;
     g.launches = 0;
     for (double& v : g.timing) v = 0.0;
-    cudaStream_t st = g.stream;
+    CK(cudaEventRecord(g.ev[0], g.stream));
+    return FREDEC_OK;
+}
 
-    CK(cudaEventRecord(g.ev[0], st));
+// stage inputs, orthogonalise + pack (prep kernel), scan.  z_out may be a host pointer, a
+// device pointer, or nullptr (library-owned device buffer, e.g. when only peaks are wanted).
+int enqueue_series(Call& c, const double* t, const double* x, const double* w, int64_t B, int64_t N,
+                   const double* base_funcs, int32_t d, double f0, double df, int64_t K, double* z_out,
+                   bool with_scan)
+{
+    cudaStream_t st = g.stream;
+    int rc;
     const double *dt, *dx, *dw, *dbase;
     const size_t BN = (size_t)B * N;
     if ((rc = stage_in(t, BN, g.in_t, &dt))) return rc;
@@ -249,14 +262,19 @@ int run_series(const double* t, const double* x, const double* w, int64_t B, int
     g.launches += 1;
     CK(cudaEventRecord(g.ev[2], st));
 
-    double* dz = nullptr;
-    double* hz = nullptr;
     if (with_scan) {
-        if ((rc = stage_out(z_out, (size_t)B * K, g.out_z, &dz, &hz))) return rc;
+        c.z_count = (size_t)B * K;
+        if (z_out == nullptr) {
+            CK(g.out_z.reserve(c.z_count * 8));
+            c.dz = g.out_z.as<double>();
+            c.hz = nullptr;
+        } else if ((rc = stage_out(z_out, c.z_count, g.out_z, &c.dz, &c.hz))) {
+            return rc;
+        }
         ScanParams sp;
         sp.rec = g.rec.as<double>();
         sp.info = g.info.as<SeriesInfo>();
-        sp.z = dz;
+        sp.z = c.dz;
         sp.N = N; sp.K = K;
         const int64_t runs = (K + pl.R - 1) / pl.R;
         sp.Kpad = runs * pl.R;
@@ -275,49 +293,20 @@ int run_series(const double* t, const double* x, const double* w, int64_t B, int
         }
     }
     CK(cudaEventRecord(g.ev[3], st));
-    if (hz) CK(cudaMemcpyAsync(hz, dz, (size_t)B * K * 8, cudaMemcpyDeviceToHost, st));
-    CK(cudaMemcpyAsync(g.h_info.p, g.info.p, (size_t)B * sizeof(SeriesInfo), cudaMemcpyDeviceToHost, st));
-    CK(cudaEventRecord(g.ev[4], st));
-    CK(cudaStreamSynchronize(st));
-
-    g.timing[0] = ev_ms(1, 2);
-    g.timing[1] = ev_ms(2, 3);
-    g.timing[3] = ev_ms(0, 4);
-    const SeriesInfo* hi = static_cast<const SeriesInfo*>(g.h_info.p);
-    for (int64_t b = 0; b < B; ++b)
-        if (hi[b].status != 0) return hi[b].status;
-    if (chi2_out) {
-        if (on_device(chi2_out)) {
-            double* tmp = static_cast<double*>(std::malloc((size_t)B * 8));
-            if (!tmp) return FREDEC_EINVAL;
-            for (int64_t b = 0; b < B; ++b) tmp[b] = hi[b].chi2_base;
-            cudaError_t e = cudaMemcpy(chi2_out, tmp, (size_t)B * 8, cudaMemcpyHostToDevice);
-            std::free(tmp);
-            CK(e);
-        } else {
-            for (int64_t b = 0; b < B; ++b) chi2_out[b] = hi[b].chi2_base;
-        }
-    }
+    c.B = B;
+    c.has_series = true;
     return FREDEC_OK;
 }
 
-int run_topk(const double* z, int64_t B, int64_t K, int32_t k, int64_t* idx_out, int* first_count)
+// peaks of the DEVICE array dz [B][K]
+int enqueue_topk(Call& c, const double* dz, int64_t B, int64_t K, int32_t k, int64_t* idx_out)
 {
-    if (!z || !idx_out || B < 1 || B > 65535 || K < 1 || k < 1 || (int64_t)k > K || k > FREDEC_TOPK_MAX)
-        return FREDEC_EINVAL;
-    int rc = ensure_ready();
-    if (rc) return rc;
-    g.launches = 0;
-    for (double& v : g.timing) v = 0.0;
     cudaStream_t st = g.stream;
-    CK(cudaEventRecord(g.ev[0], st));
-    const double* dz;
-    if ((rc = stage_in(z, (size_t)B * K, g.in_z, &dz))) return rc;
-    int64_t *didx, *hidx;
-    if ((rc = stage_out(idx_out, (size_t)B * k, g.out_idx, &didx, &hidx))) return rc;
-
+    int rc;
+    c.idx_count = (size_t)B * k;
+    if ((rc = stage_out(idx_out, c.idx_count, g.out_idx, &c.didx, &c.hidx))) return rc;
     TopkParams tp;
-    tp.z = dz; tp.idx_out = didx; tp.K = K; tp.k = k;
+    tp.z = dz; tp.idx_out = c.didx; tp.K = K; tp.k = k;
     tp.nblk = topk_pick_nblk(B, K, g.sm_count);
     CK(g.count.reserve((size_t)B * sizeof(int)));
     CK(g.h_count.reserve((size_t)B * sizeof(int)));
@@ -329,19 +318,112 @@ int run_topk(const double* z, int64_t B, int64_t K, int32_t k, int64_t* idx_out,
         tp.part_z = g.part_z.as<double>();
         tp.part_i = g.part_i.as<int64_t>();
     }
-    CK(cudaEventRecord(g.ev[1], st));
+    CK(cudaEventRecord(g.ev[4], st));
     int nl = 0;
     CK(launch_topk(tp, B, st, &nl));
-    g.launches = nl;
-    CK(cudaEventRecord(g.ev[3], st));
-    if (hidx) CK(cudaMemcpyAsync(hidx, didx, (size_t)B * k * 8, cudaMemcpyDeviceToHost, st));
-    CK(cudaMemcpyAsync(g.h_count.p, g.count.p, (size_t)B * sizeof(int), cudaMemcpyDeviceToHost, st));
-    CK(cudaEventRecord(g.ev[4], st));
-    CK(cudaStreamSynchronize(st));
-    g.timing[2] = ev_ms(1, 3);
-    g.timing[3] = ev_ms(0, 4);
-    *first_count = static_cast<const int*>(g.h_count.p)[0];
+    g.launches += nl;
+    CK(cudaEventRecord(g.ev[5], st));
+    c.B = B;
+    c.has_topk = true;
     return FREDEC_OK;
+}
+
+// copies results out, synchronises once, reads statuses; *first_count = peaks of series 0
+int finish_call(Call& c, int* first_count)
+{
+    cudaStream_t st = g.stream;
+    if (c.hz) CK(cudaMemcpyAsync(c.hz, c.dz, c.z_count * 8, cudaMemcpyDeviceToHost, st));
+    if (c.hidx) CK(cudaMemcpyAsync(c.hidx, c.didx, c.idx_count * 8, cudaMemcpyDeviceToHost, st));
+    if (c.has_series)
+        CK(cudaMemcpyAsync(g.h_info.p, g.info.p, (size_t)c.B * sizeof(SeriesInfo), cudaMemcpyDeviceToHost, st));
+    if (c.has_topk)
+        CK(cudaMemcpyAsync(g.h_count.p, g.count.p, (size_t)c.B * sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaEventRecord(g.ev[6], st));
+    CK(cudaStreamSynchronize(st));
+    if (c.has_series) {
+        g.timing[0] = ev_ms(1, 2);
+        g.timing[1] = ev_ms(2, 3);
+    }
+    if (c.has_topk) g.timing[2] = ev_ms(4, 5);
+    g.timing[3] = ev_ms(0, 6);
+    if (c.has_series) {
+        const SeriesInfo* hi = static_cast<const SeriesInfo*>(g.h_info.p);
+        for (int64_t b = 0; b < c.B; ++b)
+            if (hi[b].status != 0) return hi[b].status;
+    }
+    if (c.has_topk && first_count) *first_count = static_cast<const int*>(g.h_count.p)[0];
+    return FREDEC_OK;
+}
+
+int check_grid_args(double f0, double df, int64_t K)
+{
+    if (K < 1 || !(df > 0.0) || !(f0 >= 0.0) || !std::isfinite(f0) || !std::isfinite(df)) return FREDEC_EINVAL;
+    if (!std::isfinite(f0 + df * (double)K)) return FREDEC_EINVAL;
+    return FREDEC_OK;
+}
+
+int check_topk_args(int64_t B, int64_t K, int32_t k)
+{
+    if (B < 1 || B > 65535 || K < 1 || k < 1 || (int64_t)k > K || k > FREDEC_TOPK_MAX) return FREDEC_EINVAL;
+    return FREDEC_OK;
+}
+
+int do_scan(const double* t, const double* x, const double* w, int64_t B, int64_t N, const double* base_funcs,
+            int32_t d, double f0, double df, int64_t K, double* z_out, int32_t k, int64_t* idx_out, bool want_topk)
+{
+    int rc = check_series_args(t, x, w, B, N, base_funcs, d);
+    if (rc) return rc;
+    if ((rc = check_grid_args(f0, df, K))) return rc;
+    if (want_topk) {
+        if (!idx_out) return FREDEC_EINVAL;
+        if ((rc = check_topk_args(B, K, k))) return rc;
+    } else if (!z_out) {
+        return FREDEC_EINVAL;
+    }
+    if ((rc = begin_call())) return rc;
+    Call c;
+    if ((rc = enqueue_series(c, t, x, w, B, N, base_funcs, d, f0, df, K, z_out, true))) return rc;
+    if (want_topk && (rc = enqueue_topk(c, c.dz, B, K, k, idx_out))) return rc;
+    int count = 0;
+    if ((rc = finish_call(c, &count))) return rc;
+    return (want_topk && B == 1) ? count : FREDEC_OK;
+}
+
+int do_chi2(const double* t, const double* x, const double* w, int64_t B, int64_t N, const double* base_funcs,
+            int32_t d, double* chi2_out)
+{
+    int rc = check_series_args(t, x, w, B, N, base_funcs, d);
+    if (rc) return rc;
+    if (!chi2_out) return FREDEC_EINVAL;
+    if ((rc = begin_call())) return rc;
+    Call c;
+    if ((rc = enqueue_series(c, t, x, w, B, N, base_funcs, d, 0.0, 1.0, 1, nullptr, false))) return rc;
+    if ((rc = finish_call(c, nullptr))) return rc;
+    const SeriesInfo* hi = static_cast<const SeriesInfo*>(g.h_info.p);
+    if (on_device(chi2_out)) {
+        double* tmp = static_cast<double*>(std::malloc((size_t)B * 8));
+        if (!tmp) return FREDEC_EINVAL;
+        for (int64_t b = 0; b < B; ++b) tmp[b] = hi[b].chi2_base;
+        cudaError_t e = cudaMemcpy(chi2_out, tmp, (size_t)B * 8, cudaMemcpyHostToDevice);
+        std::free(tmp);
+        CK(e);
+    } else {
+        for (int64_t b = 0; b < B; ++b) chi2_out[b] = hi[b].chi2_base;
+    }
+    return FREDEC_OK;
+}
+
+int do_topk(const double* z, int64_t B, int64_t K, int32_t k, int64_t* idx_out, int* first_count)
+{
+    if (!z || !idx_out) return FREDEC_EINVAL;
+    int rc = check_topk_args(B, K, k);
+    if (rc) return rc;
+    if ((rc = begin_call())) return rc;
+    const double* dz;
+    if ((rc = stage_in(z, (size_t)B * K, g.in_z, &dz))) return rc;
+    Call c;
+    if ((rc = enqueue_topk(c, dz, B, K, k, idx_out))) return rc;
+    return finish_call(c, first_count);
 }
 
 }  // namespace
@@ -351,38 +433,50 @@ extern "C" {
 int fredec_scan(const double* t, const double* x, const double* w, int64_t N, const double* base_funcs,
                 int32_t d, double f0, double df, int64_t K, double* z_out)
 {
-    return run_series(t, x, w, 1, N, base_funcs, d, f0, df, K, z_out, nullptr, true);
+    return do_scan(t, x, w, 1, N, base_funcs, d, f0, df, K, z_out, 0, nullptr, false);
 }
 
 int fredec_scan_batched(const double* t, const double* x, const double* w, int64_t B, int64_t N,
                         const double* base_funcs, int32_t d, double f0, double df, int64_t K, double* z_out)
 {
-    return run_series(t, x, w, B, N, base_funcs, d, f0, df, K, z_out, nullptr, true);
+    return do_scan(t, x, w, B, N, base_funcs, d, f0, df, K, z_out, 0, nullptr, false);
+}
+
+int fredec_scan_topk(const double* t, const double* x, const double* w, int64_t N, const double* base_funcs,
+                     int32_t d, double f0, double df, int64_t K, double* z_out, int32_t k, int64_t* idx_out)
+{
+    return do_scan(t, x, w, 1, N, base_funcs, d, f0, df, K, z_out, k, idx_out, true);
+}
+
+int fredec_scan_topk_batched(const double* t, const double* x, const double* w, int64_t B, int64_t N,
+                             const double* base_funcs, int32_t d, double f0, double df, int64_t K,
+                             double* z_out, int32_t k, int64_t* idx_out)
+{
+    return do_scan(t, x, w, B, N, base_funcs, d, f0, df, K, z_out, k, idx_out, true);
 }
 
 int fredec_chi2_base(const double* t, const double* x, const double* w, int64_t N, const double* base_funcs,
                      int32_t d, double* chi2_base_out)
 {
-    return run_series(t, x, w, 1, N, base_funcs, d, 0.0, 1.0, 1, nullptr, chi2_base_out, false);
+    return do_chi2(t, x, w, 1, N, base_funcs, d, chi2_base_out);
 }
 
 int fredec_chi2_base_batched(const double* t, const double* x, const double* w, int64_t B, int64_t N,
                              const double* base_funcs, int32_t d, double* chi2_base_out)
 {
-    return run_series(t, x, w, B, N, base_funcs, d, 0.0, 1.0, 1, nullptr, chi2_base_out, false);
+    return do_chi2(t, x, w, B, N, base_funcs, d, chi2_base_out);
 }
 
 int fredec_topk(const double* z, int64_t K, int32_t k, int64_t* idx_out)
 {
     int count = 0;
-    int rc = run_topk(z, 1, K, k, idx_out, &count);
+    int rc = do_topk(z, 1, K, k, idx_out, &count);
     return rc < 0 ? rc : count;
 }
 
 int fredec_topk_batched(const double* z, int64_t B, int64_t K, int32_t k, int64_t* idx_out)
 {
-    int count = 0;
-    return run_topk(z, B, K, k, idx_out, &count);
+    return do_topk(z, B, K, k, idx_out, nullptr);
 }
 
 int fredec_set_stream(void* cuda_stream)
