@@ -13,7 +13,7 @@ namespace fredec {
 // (cp.async.bulk and LDS.128 alignment).
 //
 //   [0] t'      centred time t_i - (t_min + t_max)/2           (S10: z is origin-invariant)
-//   [1] 0       spare
+//   [1] 2 cos of 2 pi frac(df * t')           : coefficient of the two-term recurrence
 //   [2] cos, [3] sin of 2 pi frac(df * t')      : one grid step for this observation
 //   [4] cos, [5] sin of 2 pi frac(R * df * t')  : one RUN step (R grid steps)
 //   [6] w_i     weight                                          (0 in passes > 0)

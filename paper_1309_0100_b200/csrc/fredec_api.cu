@@ -176,7 +176,8 @@ ScanPlan plan_scan(int64_t B, int64_t N, int d, int64_t K)
     while (FW < 4 && FW * 2 * S <= 8 && fwarps / (FW * 2) >= 2 * (int64_t)g.sm_count) FW *= 2;
     pl.S = S;
     pl.FW = FW;
-    int TI = rec_stride(pl.NB) <= 16 ? 128 : 64;
+    int TI = 4096 / (FW * 32);   // seeds: J x (TI+1) x 16 B ~ 64 KB per CTA
+    if (TI > 128) TI = 128;
     if (N < TI) TI = (int)((N + S - 1) / S * S);
     pl.TI = TI;
     return pl;

@@ -148,7 +148,7 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p)
             sincospi(2.0 * frac_prod(dfR, tc), &sR, &cR);
             const double wi = w[i];
             r[0] = tc;
-            r[1] = 0.0;
+            r[1] = 2.0 * c1;
             r[2] = c1;
             r[3] = s1;
             r[4] = cR;

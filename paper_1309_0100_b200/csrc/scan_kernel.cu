@@ -9,14 +9,25 @@
 // and solves the 2x2 Schur complement (the last two steps of the Cholesky forward
 // substitution of PAPER.md:175/183) in the epilogue: z = a_d^2 + a_{d+1}^2.
 //
-// Work decomposition: a thread owns a RUN of R consecutive grid frequencies and keeps their
-// R*(4+2NB) sums in registers.  Observation records are staged tile by tile into shared
-// memory with 1-D TMA bulk copies (cp.async.bulk + mbarrier, double buffered) and read as
-// warp-broadcast LDS.128.  For each observation the thread seeds (cos, sin) at its first
-// frequency from an exactly range-reduced phase and then advances along the frequency axis
-// with the rotation recurrence (cos, sin) <- (cos, sin) x (cos d_i, sin d_i).
-// No per-pair sincos.  Partial sums of warps that split the observations of a tile are
-// combined in a fixed order through shared memory (bitwise reproducible).
+// Work decomposition.  A thread owns a RUN of R consecutive grid frequencies and keeps their
+// R*(4+2NB) sums in registers; a CTA owns J = 32*FW consecutive runs.  Observation records
+// are staged tile by tile into shared memory with 1-D TMA bulk copies (cp.async.bulk +
+// mbarrier, double buffered) and read as warp-broadcast LDS.128.  Per tile:
+//
+//   phase A (seeds)  e^{i phi} at the FIRST frequency of every run, for every observation of
+//                    the tile, into shared memory.  Along the run axis consecutive seeds
+//                    differ by the per-observation rotation e^{i 2 pi R df t'}: every
+//                    kSeedChain-th seed is evaluated from the exactly range-reduced phase
+//                    (frac(f t') by an FMA split, then sincospi), the ones in between by the
+//                    FP64 rotation recurrence.  Cost: ~5 FP64 instructions per seed.
+//   phase B (sums)   each thread walks the tile's observations; for each it loads its seed,
+//                    makes the second starting value with one rotation by e^{i 2 pi df t'}
+//                    and then advances along the frequency axis with the two-term form of
+//                    the rotation recurrence, c_{r+1} = 2 cos(d) c_r - c_{r-1} (same for s),
+//                    2 FMA per step, re-seeded every R steps.  No per-pair sincos.
+//
+// Partial sums of warps that split the observations of a tile are combined in a fixed order
+// through shared memory (bitwise reproducible run to run).
 #include "scan_kernel.cuh"
 
 namespace fredec {
@@ -59,26 +70,33 @@ struct Acc {
     }
 };
 
+// one thread's share of phase A: two independent chains of kSeedChain seeds
+constexpr int kSeedChain = 16;
+
 template <int R, int NB>
 __global__ void __launch_bounds__(kMaxScanThreads, 1) scan_kernel(ScanParams p)
 {
     constexpr int RS = rec_stride(NB);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t bar[2];
-    double* const tile_buf = reinterpret_cast<double*>(smem_raw);
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int FW = p.FW, S = p.S, TI = p.TI;
+    const int J = FW * 32, T = J * S;
+    const int SROW = TI + 1;  // seed row stride in double2 (odd: conflict-free both ways)
+    double* const tile_buf = reinterpret_cast<double*>(smem_raw);                      // [2][TI][RS]
+    double2* const seeds = reinterpret_cast<double2*>(tile_buf + (size_t)2 * TI * RS);  // [J][SROW]
+
     const int fw = wid % FW, sp = wid / FW;
+    const int jrun = fw * 32 + lane;  // this thread's run within the CTA
     const int64_t b = blockIdx.y;
     const SeriesInfo info = p.info[b];
     if (info.status != 0) return;  // uniform over the CTA; the host reports the error
 
     const int64_t N = p.N, K = p.K;
-    const int64_t run = (int64_t)blockIdx.x * (FW * 32) + fw * 32 + lane;
-    const int64_t k0 = run * R;
+    const int64_t run0 = (int64_t)blockIdx.x * J;  // first run of the CTA
+    const int64_t k0 = (run0 + jrun) * R;
     const bool active = k0 < K;
-    const double fk0 = fma((double)k0, p.df, p.f0);  // S1: the run starts on fl(f0 + k0 df)
     const double* rec = p.rec + ((b * p.n_pass + p.pass) * N) * RS;
 
     const int ntiles = (int)((N + TI - 1) / TI);
@@ -102,18 +120,57 @@ __global__ void __launch_bounds__(kMaxScanThreads, 1) scan_kernel(ScanParams p)
     acc.clear();
 
     const int rows_per_split = TI / S;
+    const int nseg = J / kSeedChain;  // chains per observation
     for (int tile = 0; tile < ntiles; ++tile) {
         if (tid == 0 && tile + 1 < ntiles) issue(tile + 1);  // stage (tile+1)&1 was released by the
                                                              // __syncthreads that ended tile-1
         mbar_wait(&bar[tile & 1], (uint32_t)((tile >> 1) & 1));
         const int rows = (int)min((int64_t)TI, N - (int64_t)tile * TI);
+        const double* tb = tile_buf + (size_t)(tile & 1) * TI * RS;
+
+        // ---- phase A: seeds[j][i] = (cos, sin)(2 pi f_{(run0+j)R} t'_i) -----------------------
+        // chain c = (segment g, observation i), i fastest => conflict-free STS.128
+        const int nchains = nseg * rows;
+        for (int c0 = tid; c0 < nchains; c0 += 2 * T) {
+            const int c1 = c0 + T;
+            const bool two = c1 < nchains;
+            const int ia = c0 % rows, ga = c0 / rows;
+            const int ib = two ? c1 % rows : ia, gb = two ? c1 / rows : ga;
+            const double2* ra = reinterpret_cast<const double2*>(tb + (size_t)ia * RS);
+            const double2* rb = reinterpret_cast<const double2*>(tb + (size_t)ib * RS);
+            const double ta = ra[0].x, tbb = rb[0].x;
+            const double2 Ga = ra[2], Gb = rb[2];  // (cos, sin) of one run step
+            // exact seeds at the head of each chain (S1: f = fl(f0 + k df))
+            const double fa = fma((double)((run0 + (int64_t)ga * kSeedChain) * R), p.df, p.f0);
+            const double fb = fma((double)((run0 + (int64_t)gb * kSeedChain) * R), p.df, p.f0);
+            double ca, sa, cb, sb;
+            sincospi(2.0 * frac_prod(fa, ta), &sa, &ca);
+            sincospi(2.0 * frac_prod(fb, tbb), &sb, &cb);
+            double2* da = seeds + (size_t)(ga * kSeedChain) * SROW + ia;
+            double2* db = seeds + (size_t)(gb * kSeedChain) * SROW + ib;
+#pragma unroll
+            for (int q = 0; q < kSeedChain; ++q) {
+                da[(size_t)q * SROW] = make_double2(ca, sa);
+                if (two) db[(size_t)q * SROW] = make_double2(cb, sb);
+                if (q + 1 < kSeedChain) {
+                    const double na = fma(ca, Ga.x, -(sa * Ga.y));
+                    const double ma = fma(sa, Ga.x, ca * Ga.y);
+                    const double nb = fma(cb, Gb.x, -(sb * Gb.y));
+                    const double mb = fma(sb, Gb.x, cb * Gb.y);
+                    ca = na; sa = ma; cb = nb; sb = mb;
+                }
+            }
+        }
+        __syncthreads();
+
+        // ---- phase B: accumulate this warp's share of the tile --------------------------------
         const int i_begin = sp * rows_per_split;
         const int i_end = min(rows, i_begin + rows_per_split);
-        const double* tb = tile_buf + (size_t)(tile & 1) * TI * RS;
         if (active) {
+            const double2* myseed = seeds + (size_t)jrun * SROW;
             for (int i = i_begin; i < i_end; ++i) {
                 const double2* r2 = reinterpret_cast<const double2*>(tb + (size_t)i * RS);
-                const double2 h0 = r2[0];  // t', -
+                const double2 h0 = r2[0];  // t', 2 cos d
                 const double2 h1 = r2[1];  // cos d, sin d
                 const double2 h3 = r2[3];  // w, y
                 double pj[NB > 0 ? NB : 1];
@@ -123,30 +180,31 @@ __global__ void __launch_bounds__(kMaxScanThreads, 1) scan_kernel(ScanParams p)
                     pj[j] = q.x;
                     if (j + 1 < NB) pj[j + 1] = q.y;
                 }
-                // a5: seed at the run's first frequency from the exactly reduced phase
-                double c, s;
-                sincospi(2.0 * frac_prod(fk0, h0.x), &s, &c);
-                const double cd = h1.x, sd = h1.y, w = h3.x, y = h3.y;
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    // a6: accumulate
-                    acc.YC[r] = fma(y, c, acc.YC[r]);
-                    acc.YS[r] = fma(y, s, acc.YS[r]);
-                    const double u = w * c;
-                    acc.CC[r] = fma(u, c, acc.CC[r]);
-                    acc.CS[r] = fma(u, s, acc.CS[r]);
+                const double2 sd = myseed[i];
+                const double k2 = h0.y, w = h3.x, y = h3.y;
+                double cm = sd.x, sm = sd.y;                    // r = 0
+                double c = fma(cm, h1.x, -(sm * h1.y));         // r = 1: one rotation by d
+                double s = fma(sm, h1.x, cm * h1.y);
+                auto accumulate = [&](int r, double cc, double ss) {
+                    acc.YC[r] = fma(y, cc, acc.YC[r]);
+                    acc.YS[r] = fma(y, ss, acc.YS[r]);
+                    const double u = w * cc;
+                    acc.CC[r] = fma(u, cc, acc.CC[r]);
+                    acc.CS[r] = fma(u, ss, acc.CS[r]);
 #pragma unroll
                     for (int j = 0; j < NB; ++j) {
-                        acc.A[r][j] = fma(pj[j], c, acc.A[r][j]);
-                        acc.B[r][j] = fma(pj[j], s, acc.B[r][j]);
+                        acc.A[r][j] = fma(pj[j], cc, acc.A[r][j]);
+                        acc.B[r][j] = fma(pj[j], ss, acc.B[r][j]);
                     }
-                    // a7: rotate to the next grid frequency
-                    if (r + 1 < R) {
-                        const double cn = fma(c, cd, -(s * sd));
-                        const double sn = fma(s, cd, c * sd);
-                        c = cn;
-                        s = sn;
-                    }
+                };
+                accumulate(0, cm, sm);
+                accumulate(1, c, s);
+#pragma unroll
+                for (int r = 2; r < R; ++r) {
+                    const double cn = fma(k2, c, -cm);  // a7: c_{r+1} = 2 cos(d) c_r - c_{r-1}
+                    const double sn = fma(k2, s, -sm);
+                    cm = c; sm = s; c = cn; s = sn;
+                    accumulate(r, c, s);
                 }
             }
         }
@@ -156,11 +214,11 @@ __global__ void __launch_bounds__(kMaxScanThreads, 1) scan_kernel(ScanParams p)
     // ---- a8: combine the observation split in a fixed order ------------------------------
     if (S > 1) {
         double* red = tile_buf;  // every bulk copy has completed and been consumed
-        const int nthr_f = FW * 32, col = fw * 32 + lane;
+        const int col = jrun;
         for (int q = 1; q < S; ++q) {
-            if (sp == q) acc.for_each([&](double& v, int a) { red[a * nthr_f + col] = v; });
+            if (sp == q) acc.for_each([&](double& v, int a) { red[a * J + col] = v; });
             __syncthreads();
-            if (sp == 0) acc.for_each([&](double& v, int a) { v += red[a * nthr_f + col]; });
+            if (sp == 0) acc.for_each([&](double& v, int a) { v += red[a * J + col]; });
             __syncthreads();
         }
     }
@@ -248,8 +306,9 @@ cudaError_t launch_one(const ScanParams& p, int64_t B, cudaStream_t stream)
 size_t scan_smem_bytes(int R, int NB, const ScanParams& p)
 {
     const size_t tiles = 2 * (size_t)p.TI * rec_stride(NB) * 8;
+    const size_t seeds = (size_t)p.FW * 32 * (p.TI + 1) * 16;
     const size_t red = p.S > 1 ? (size_t)R * (4 + 2 * NB) * p.FW * 32 * 8 : 0;
-    return tiles > red ? tiles : red;
+    return (tiles > red ? tiles : red) + seeds;
 }
 
 #define FREDEC_SCAN_CONFIGS(X) \
