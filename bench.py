@@ -40,12 +40,17 @@ WORKLOAD = "config4 survey: N=10000 obs x K=2000000 freqs, d=2 (offset+trend), t
 FP64_LANES_PER_SM = 64
 L2_FLUSH_BYTES = 256 << 20
 ORACLE_SAMPLE_K = 20_000          # grid points of config 4 the CPU legs time per step
+# dram__bytes_read.sum + dram__bytes_write.sum of one scan_kernel launch on config 4, from the
+# `ncu --set full` capture summarised in profiles/r1_scan_kernel_ncu.md (849 920 B read, 0 B written:
+# the 16 MB periodogram is still in L2 when the kernel ends).  Algorithmic bytes: 0.8 MB + 16 MB.
+SCAN_DRAM_TRAFFIC_BYTES = 849_920
 
 
 def flops_per_pair(d: int) -> int:
-    """Algorithmic FP64 flops per (frequency, observation) pair: accumulate
-    (4+2d) FMA + 1 MUL, rotate 2 MUL + 2 FMA."""
-    return 15 + 4 * d
+    """Algorithmic FP64 flops per (frequency, observation) pair, for the
+    two-term recurrence the kernel executes: accumulate (4+2d) FMA + 1 MUL = 9+4d, advance
+    2 FMA = 4.  (The rotation form would be 15+4d; flops that are not executed are not credited.)"""
+    return 13 + 4 * d
 
 
 class ClockSampler:
@@ -303,8 +308,9 @@ def main_ours(args):
                    "peaks": peaks},
         "kernel_ms": {"prep": kern["prep_ms"] / args.steps, "scan": scan_ms, "topk": kern["topk_ms"] / args.steps},
         "fraction_of_fp64_peak": achieved / peak_nominal,
+        "fraction_of_fp64_peak_rotation_form_equivalent": achieved / peak_nominal * (15 + 4 * wl.d) / F,
         "roofline": {"bound": "alu", "kernel": "scan_kernel", "achieved": achieved, "peak": peak_nominal,
-                     "unit": "TFLOP/s", "frac": achieved / peak_nominal, "traffic": None,
+                     "unit": "TFLOP/s", "frac": achieved / peak_nominal, "traffic": SCAN_DRAM_TRAFFIC_BYTES,
                      "flops_per_pair": F, "peak_source": f"nominal: {sm_count} SMs x {FP64_LANES_PER_SM} FP64 FMA "
                      "lanes x 2 x 1.965 GHz (DESIGN.md section 6)",
                      "peak_measured_dfma": peak_tf, "frac_of_measured_dfma": achieved / peak_tf},

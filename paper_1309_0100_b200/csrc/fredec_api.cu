@@ -161,7 +161,11 @@ ScanPlan plan_scan(int64_t B, int64_t N, int d, int64_t K)
 {
     ScanPlan pl;
     if (d <= 3) {
+#ifdef FREDEC_PLAN_R_SMALL
+        pl.R = FREDEC_PLAN_R_SMALL; pl.NB = d; pl.n_pass = 1;
+#else
         pl.R = 8; pl.NB = d; pl.n_pass = 1;
+#endif
     } else if (d <= 9) {
         pl.R = 4; pl.NB = d; pl.n_pass = 1;
     } else {
@@ -170,13 +174,17 @@ ScanPlan plan_scan(int64_t B, int64_t N, int d, int64_t K)
     const int64_t runs = (K + pl.R - 1) / pl.R;
     const int64_t fwarps = (runs + 31) / 32 * B;   // warps if every run had its own lane once
     const int64_t target = (int64_t)g.sm_count * 8;
+    const int max_warps = scan_max_warps();
     int S = 1;
-    while (S < 8 && fwarps * (S * 2) <= target && N / (S * 2) >= 16) S *= 2;
+    while (S * 2 <= max_warps && fwarps * (S * 2) <= target && N / (S * 2) >= 16) S *= 2;
     int FW = 1;
-    while (FW < 4 && FW * 2 * S <= 8 && fwarps / (FW * 2) >= 2 * (int64_t)g.sm_count) FW *= 2;
+    while (FW < 4 && FW * 2 * S <= max_warps && fwarps / (FW * 2) >= 2 * (int64_t)g.sm_count) FW *= 2;
     pl.S = S;
     pl.FW = FW;
-    int TI = 4096 / (FW * 32);   // seeds: J x (TI+1) x 16 B ~ 64 KB per CTA
+#ifndef FREDEC_PLAN_SEED_ELEMS
+#define FREDEC_PLAN_SEED_ELEMS 4096
+#endif
+    int TI = FREDEC_PLAN_SEED_ELEMS / (FW * 32);   // seeds: J x (TI+1) x 16 B ~ 64 KB per CTA
     if (TI > 128) TI = 128;
     if (N < TI) TI = (int)((N + S - 1) / S * S);
     pl.TI = TI;

@@ -19,6 +19,7 @@ struct ScanParams {
 
 // Supported (R, NB) instantiations; returns false if (R, NB) is not built.
 bool scan_config_supported(int R, int NB);
+int scan_max_warps();  // FW * S may not exceed this
 size_t scan_smem_bytes(int R, int NB, const ScanParams& p);
 cudaError_t launch_scan(int R, int NB, const ScanParams& p, int64_t B, cudaStream_t stream);
 
