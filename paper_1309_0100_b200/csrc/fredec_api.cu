@@ -11,6 +11,7 @@
 #include "peak_kernel.cuh"
 #include "prep_kernel.cuh"
 #include "scan_kernel.cuh"
+#include "scan_mma_kernel.cuh"
 #include "topk_kernel.cuh"
 
 using namespace fredec;
@@ -74,7 +75,7 @@ struct State {
     cudaStream_t stream = nullptr;
     cudaEvent_t ev[kNumEvents] = {};
     DevBuf in_t, in_x, in_w, in_base, in_z, out_z, out_idx, out_chi2;
-    DevBuf rec, psi, xt, info, ws, part_z, part_i, count, sink;
+    DevBuf rec, tab, srec, psi, xt, info, ws, part_z, part_i, count, sink;
     HostBuf h_info, h_count;
     int last_cuda = 0;
     double timing[4] = {0, 0, 0, 0};
@@ -237,6 +238,80 @@ int begin_call()
     return FREDEC_OK;
 }
 
+// orthogonalise (prep kernel), table kernel, MMA scan; inputs already on the device
+int enqueue_series_mma(Call& c, const double* dt, const double* dx, const double* dw, const double* dbase, int64_t B,
+                       int64_t N, int32_t d, double f0, double df, int64_t K, double* z_out)
+{
+    cudaStream_t st = g.stream;
+    int rc;
+    const size_t BN = (size_t)B * N;
+    const int NB = d <= kMmaMaxNB ? d : 8;
+    const int n_pass = d <= kMmaMaxNB ? 1 : (d + 7) / 8;
+    const MmaScanConfig cfg = mma_scan_config(NB);
+    const int R = 2 * cfg.H;
+    const int64_t G4 = (N + 3) / 4;
+    const int64_t U = (K + 8 * R - 1) / (8 * R);
+
+    CK(g.psi.reserve(BN * (size_t)(d > 0 ? d : 1) * 8));
+    CK(g.xt.reserve(BN * 8));
+    CK(g.info.reserve((size_t)B * sizeof(SeriesInfo)));
+    CK(g.h_info.reserve((size_t)B * sizeof(SeriesInfo)));
+    CK(g.tab.reserve((size_t)B * n_pass * G4 * mma_group_doubles(cfg.H, NB) * 8));
+    CK(g.srec.reserve((size_t)B * G4 * 4 * sizeof(SeedRec)));
+
+    PrepParams pp;
+    pp.t = dt; pp.x = dx; pp.w = dw; pp.base = dbase;
+    pp.psi = g.psi.as<double>(); pp.xt = g.xt.as<double>();
+    pp.rec = nullptr;
+    pp.info = g.info.as<SeriesInfo>();
+    pp.N = N; pp.d = d; pp.NB = NB; pp.n_pass = n_pass; pp.R = R; pp.df = df;
+    CK(cudaEventRecord(g.ev[1], st));
+    CK(launch_prep(pp, B, st));
+    TableParams tp;
+    tp.t = dt; tp.w = dw; tp.psi = g.psi.as<double>(); tp.xt = g.xt.as<double>();
+    tp.info = g.info.as<SeriesInfo>();
+    tp.tab = g.tab.as<double>(); tp.srec = g.srec.as<SeedRec>();
+    tp.N = N; tp.G4 = G4; tp.d = d; tp.NB = NB; tp.n_pass = n_pass; tp.H = cfg.H; tp.df = df;
+    CK(launch_table(tp, B, st));
+    g.launches += 2;
+    CK(cudaEventRecord(g.ev[2], st));
+
+    c.z_count = (size_t)B * K;
+    if (z_out == nullptr) {
+        CK(g.out_z.reserve(c.z_count * 8));
+        c.dz = g.out_z.as<double>();
+        c.hz = nullptr;
+    } else if ((rc = stage_out(z_out, c.z_count, g.out_z, &c.dz, &c.hz))) {
+        return rc;
+    }
+    MmaScanParams sp;
+    sp.tab = g.tab.as<double>(); sp.srec = g.srec.as<SeedRec>();
+    sp.info = g.info.as<SeriesInfo>();
+    sp.z = c.dz;
+    sp.N = N; sp.K = K; sp.Kpad = U * 8 * R;
+    sp.G4 = G4; sp.U = U; sp.T = B * U;
+    sp.f0 = f0; sp.df = df;
+    sp.n_pass = n_pass;
+    sp.grid = (int)(sp.T < (int64_t)g.sm_count ? sp.T : (int64_t)g.sm_count);
+    int TI = 4 * cfg.NW;  // phase A hands one group of 4 observations to each warp
+    while (TI < 64 && mma_scan_smem_bytes(NB, TI * 2) <= 200 * 1024 && (int64_t)TI * 2 <= G4 * 4 + 4 * cfg.NW) TI *= 2;
+    sp.TI = TI;
+    sp.ws = nullptr;
+    if (n_pass > 1) {
+        CK(g.ws.reserve((size_t)B * 7 * sp.Kpad * 8));
+        sp.ws = g.ws.as<double>();
+    }
+    for (int pass = 0; pass < n_pass; ++pass) {
+        sp.pass = pass;
+        CK(launch_mma_scan(NB, sp, st));
+        g.launches += 1;
+    }
+    CK(cudaEventRecord(g.ev[3], st));
+    c.B = B;
+    c.has_series = true;
+    return FREDEC_OK;
+}
+
 // stage inputs, orthogonalise + pack (prep kernel), scan.  z_out may be a host pointer, a
 // device pointer, or nullptr (library-owned device buffer, e.g. when only peaks are wanted).
 int enqueue_series(Call& c, const double* t, const double* x, const double* w, int64_t B, int64_t N,
@@ -251,6 +326,9 @@ int enqueue_series(Call& c, const double* t, const double* x, const double* w, i
     if ((rc = stage_in(x, BN, g.in_x, &dx))) return rc;
     if ((rc = stage_in(w, BN, g.in_w, &dw))) return rc;
     if ((rc = stage_in(base_funcs, BN * d, g.in_base, &dbase))) return rc;
+
+    static const bool use_old = std::getenv("FREDEC_SCAN_OLD") != nullptr;
+    if (with_scan && !use_old) return enqueue_series_mma(c, dt, dx, dw, dbase, B, N, d, f0, df, K, z_out);
 
     ScanPlan pl = plan_scan(B, N, d, with_scan ? K : 1);
     const int RS = rec_stride(pl.NB);
@@ -524,7 +602,7 @@ int fredec_fp64_peak(int64_t iters, double* tflops_out, double* ms_out)
 
 int fredec_shutdown(void)
 {
-    DevBuf* bufs[] = {&g.in_t, &g.in_x, &g.in_w, &g.in_base, &g.in_z, &g.out_z, &g.out_idx, &g.out_chi2, &g.rec,
+    DevBuf* bufs[] = {&g.in_t, &g.in_x, &g.in_w, &g.in_base, &g.in_z, &g.out_z, &g.out_idx, &g.out_chi2, &g.rec, &g.tab, &g.srec,
                       &g.psi,  &g.xt,   &g.info, &g.ws,      &g.part_z, &g.part_i, &g.count, &g.sink};
     for (DevBuf* b : bufs) b->release();
     g.h_info.release();

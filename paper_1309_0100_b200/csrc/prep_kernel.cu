@@ -163,7 +163,67 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p)
     }
 }
 
+// ---- a3 for the MMA scan: per-observation table and seed records --------------------------
+// One thread per observation (padded to whole groups of 4 with zero multipliers).  Layout:
+// scan_mma_kernel.cuh.
+constexpr int kTableThreads = 128;
+
+__global__ void __launch_bounds__(kTableThreads) table_kernel(TableParams p)
+{
+    const int64_t b = blockIdx.z, N = p.N;
+    const int pass = blockIdx.y;
+    const SeriesInfo info = p.info[b];
+    if (info.status != 0) return;
+    const int64_t i = (int64_t)blockIdx.x * kTableThreads + threadIdx.x;
+    if (i >= p.G4 * 4) return;
+    const bool real = i < N;
+    const int H = p.H, NT = mma_nt(H), NF = mma_nf(p.NB);
+    const double tc = real ? p.t[b * N + i] - info.t_mid : 0.0;
+    const double wi = real ? p.w[b * N + i] : 0.0;
+    if (pass == 0) {
+        SeedRec r;
+        r.t = tc;
+        sincospi(2.0 * frac_prod(p.df * (double)(16 * H), tc), &r.su, &r.cu);  // one unit = 8 runs of 2H steps
+        r.pad = 0.0;
+        p.srec[b * p.G4 * 4 + i] = r;
+    }
+    double* grp = p.tab + ((b * p.n_pass + pass) * p.G4 + i / 4) * mma_group_doubles(H, p.NB);
+    const int k = (int)(i & 3);
+    const double* psi = p.psi + b * (int64_t)p.d * N;
+    for (int h = 1; h <= H; ++h) {
+        // alpha_h = 2 pi (h - 1/2) df t' in turns, range-reduced exactly
+        const double x = frac_prod((double)(2 * h - 1) * (0.5 * p.df), tc);
+        double c1, s1, c2, s2;
+        sincospi(2.0 * x, &s1, &c1);
+        sincospi(4.0 * x, &s2, &c2);
+        const int nt = (h - 1) >> 2, n0 = 2 * ((h - 1) & 3);
+        for (int f = 0; f < NF; ++f) {
+            double m, c = c1, s = s1;
+            if (f == 0) {
+                m = (pass == 0 && real) ? wi * p.xt[b * N + i] : 0.0;
+            } else if (f == NF - 1) {
+                m = pass == 0 ? 0.5 * wi : 0.0;
+                c = c2;
+                s = s2;
+            } else {
+                const int j = pass * p.NB + (f - 1);
+                m = (j < p.d && real) ? wi * psi[(int64_t)j * N + i] : 0.0;
+            }
+            double* tile = grp + (f * NT + nt) * 32;
+            tile[n0 * 4 + k] = m * c;
+            tile[(n0 + 1) * 4 + k] = m * s;
+        }
+    }
+}
+
 }  // namespace
+
+cudaError_t launch_table(const TableParams& p, int64_t B, cudaStream_t stream)
+{
+    dim3 grid((unsigned)((p.G4 * 4 + kTableThreads - 1) / kTableThreads), (unsigned)p.n_pass, (unsigned)B);
+    table_kernel<<<grid, kTableThreads, 0, stream>>>(p);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_prep(const PrepParams& p, int64_t B, cudaStream_t stream)
 {

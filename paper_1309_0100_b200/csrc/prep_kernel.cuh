@@ -1,6 +1,7 @@
 // prep_kernel.cuh -- launch interface of the orthogonalisation / packing kernel.
 #pragma once
 #include "common.cuh"
+#include "scan_mma_kernel.cuh"
 
 namespace fredec {
 
@@ -20,6 +21,22 @@ struct PrepParams {
     int R;       // grid steps per run (power of two)
     double df;
 };
+
+// a3 for the MMA scan (scan_mma_kernel.cuh): table + seed records from the prep kernel's psi, x~
+struct TableParams {
+    const double* t;         // [B][N]
+    const double* w;         // [B][N]
+    const double* psi;       // [B][d][N] orthonormal base (prep kernel)
+    const double* xt;        // [B][N] residual x~ (prep kernel)
+    const SeriesInfo* info;  // [B]
+    double* tab;             // out [B][n_pass][G4][NF][NT][32]
+    SeedRec* srec;           // out [B][G4 * 4]
+    int64_t N, G4;
+    int d, NB, n_pass, H;
+    double df;
+};
+
+cudaError_t launch_table(const TableParams& p, int64_t B, cudaStream_t stream);
 
 cudaError_t launch_prep(const PrepParams& p, int64_t B, cudaStream_t stream);
 

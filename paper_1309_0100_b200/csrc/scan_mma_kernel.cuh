@@ -1,0 +1,56 @@
+// scan_mma_kernel.cuh -- launch interface of the frequency-scan kernel (steps a4-a10).
+#pragma once
+#include "common.cuh"
+
+namespace fredec {
+
+// Layout constants shared by the table kernel (writer) and the scan kernel (reader).
+//
+// The grid is cut into RUNS of R = 2H consecutive frequencies, symmetric about the run's
+// centre frequency f_c (half a grid step between two grid points); eight runs make a UNIT
+// (one 8-row MMA tile).  For an observation i the phase at grid point f_c +- (h - 1/2) df is
+// phi_i +- alpha_hi with phi_i = 2 pi f_c t'_i (depends on the run: a "seed") and
+// alpha_hi = 2 pi (h - 1/2) df t'_i (the same for every run: a per-observation TABLE).
+//
+// Table, per group of 4 observations: [family][column tile][32 doubles in B-fragment order],
+// families: 0 = y (w x~), 1..NB = p_j (w psi_j), NB+1 = w/2.  Column n = 2 hh + type of tile
+// nt belongs to h = 4 nt + hh + 1; type 0 = cos, 1 = sin of alpha_h (of 2 alpha_h in the
+// w family); the entry is multiplier x trig value.  Fragment order: element (k = observation
+// within the group, n = column) sits at n * 4 + k, i.e. at the lane that owns it in
+// mma.m8n8k4's B operand.
+__host__ __device__ constexpr int mma_nt(int H) { return H / 4; }
+__host__ __device__ constexpr int mma_nf(int NB) { return NB + 2; }
+__host__ __device__ constexpr int mma_group_doubles(int H, int NB) { return mma_nf(NB) * mma_nt(H) * 32; }
+
+// Per-observation seed record: t', (cos, sin) of the rotation by one unit (8 runs = 8R grid steps).
+struct __align__(32) SeedRec {
+    double t, cu, su, pad;
+};
+
+struct MmaScanParams {
+    const double* tab;       // [B][n_pass][G4][NF][NT][32]
+    const SeedRec* srec;     // [B][G4 * 4]
+    const SeriesInfo* info;  // [B]
+    double* z;               // [B][K] out
+    double* ws;              // [B][7][Kpad] partial sums between passes (nullptr if n_pass == 1)
+    int64_t N, K, Kpad;
+    int64_t G4;  // groups of 4 observations per series = ceil(N / 4)
+    int64_t U;   // units per series = ceil(K / (8 R))
+    int64_t T;   // total units = B * U
+    double f0, df;
+    int n_pass, pass;
+    int TI;    // observations per shared-memory tile (multiple of 4 * warps per CTA)
+    int grid;  // CTAs (persistent; each owns a contiguous range of units)
+};
+
+struct MmaScanConfig {
+    int H, NOCT, NW;  // half run length, units per warp and round, warps per CTA
+};
+
+// The (H, NOCT) the library is built with for NB base functions per pass (NB <= kMmaMaxNB).
+constexpr int kMmaMaxNB = 9;
+MmaScanConfig mma_scan_config(int NB);
+size_t mma_scan_smem_bytes(int NB, int TI);
+cudaError_t launch_mma_scan(int NB, const MmaScanParams& p, cudaStream_t stream);
+
+}  // namespace fredec
