@@ -293,9 +293,13 @@ int enqueue_series_mma(Call& c, const double* dt, const double* dx, const double
     sp.f0 = f0; sp.df = df;
     sp.n_pass = n_pass;
     sp.grid = (int)(sp.T < (int64_t)g.sm_count ? sp.T : (int64_t)g.sm_count);
-    int TI = 4 * cfg.NW;  // phase A hands one group of 4 observations to each warp
-    while (TI < 64 && mma_scan_smem_bytes(NB, TI * 2) <= 200 * 1024 && (int64_t)TI * 2 <= G4 * 4 + 4 * cfg.NW) TI *= 2;
-    sp.TI = TI;
+    // ring of (table tile, seeds) slots: 32 observations per slot (two groups of 4 per seed warp)
+    // if at least three slots fit in ~208 KB of shared memory, else 16; as many slots as fit
+    sp.TI = 32;
+    if ((208 * 1024) / mma_scan_slot_bytes(NB, sp.TI) < 3 || G4 <= 4) sp.TI = 16;
+    sp.NS = (int)((208 * 1024) / mma_scan_slot_bytes(NB, sp.TI));
+    if (sp.NS > kMmaMaxSlots) sp.NS = kMmaMaxSlots;
+    if (sp.NS < 2) return FREDEC_EINVAL;
     sp.ws = nullptr;
     if (n_pass > 1) {
         CK(g.ws.reserve((size_t)B * 7 * sp.Kpad * 8));

@@ -184,6 +184,7 @@ __global__ void __launch_bounds__(kTableThreads) table_kernel(TableParams p)
         SeedRec r;
         r.t = tc;
         sincospi(2.0 * frac_prod(p.df * (double)(16 * H), tc), &r.su, &r.cu);  // one unit = 8 runs of 2H steps
+        sincospi(2.0 * frac_prod(p.df * (double)(64 * H), tc), &r.s4, &r.c4);  // four units
         r.pad = 0.0;
         p.srec[b * p.G4 * 4 + i] = r;
     }

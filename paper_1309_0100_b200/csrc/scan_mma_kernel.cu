@@ -28,19 +28,26 @@
 //
 // Work decomposition.  8 runs = one UNIT (an 8-row MMA tile, 8R frequencies).  The CTA is
 // persistent and owns a contiguous range of units, processed in ROUNDS of up to
-// kNW * NOCT units of one series; within a round warp w owns up to NOCT units, whose
+// kMmaWarps * NOCT units of one series; within a round MMA warp w owns up to NOCT units, whose
 // 2 * NF * NT accumulator tiles per unit stay in registers while the round streams over all
-// observations tile by tile:
+// observations, one STEP = one tile of TI observations at a time.
 //
-//   stage   table tile + seed records, global -> shared by 1-D TMA (cp.async.bulk + mbarrier),
-//           three stages
-//   phase A seeds e^{i phi} for every (run of the round, observation of the NEXT tile) into
-//           shared memory in A-fragment order: one exact evaluation (range-reduced phase,
-//           sincospi) at the round's first unit, then one FP64 rotation per further unit
-//   phase B per 4 observations: A fragments (seeds; double-angle seeds by 4 flops), B fragments
-//           (table), 2 * NF * NT MMAs per unit
-//   a9/a10  after the last tile the thread that holds all sums of a frequency solves and stores z.
+// The CTA is warp-specialised (three warpgroups; registers moved between them with
+// setmaxnreg) around a ring of NS shared-memory slots, slot = (table tile, seeds) of one step:
 //
+//   seed warps (4, one per SM sub-partition)  wait until the MMA warps have left the slot
+//           (mbarrier "done"); one lane stages the table tile global -> shared by 1-D TMA
+//           (cp.async.bulk, mbarrier "tab"); then a5: seeds e^{i phi} for every (run of the
+//           round, observation of the tile) in A-fragment order -- one exact evaluation
+//           (range-reduced phase, sincospi) at the round's first unit, rotations by 4 units and
+//           by 1 unit for the others (four independent chains) -- and arrive on mbarrier "seed".
+//   MMA warps (8, two per sub-partition)  wait for "tab" and "seed"; per 4 observations:
+//           A fragments (seeds; double-angle seeds by 4 flops), B fragments (table),
+//           2 * NF * NT MMAs per unit; arrive on "done".  After the last tile of a round the
+//           thread that holds all sums of a frequency solves (a9) and stores z (a10).
+//
+// The seed warps run up to NS steps ahead of the MMA warps, so the latency of the seed chains
+// (which share the FP64 pipe with the MMAs) is off the MMA warps' critical path.
 // Every accumulation order is fixed, so results are bitwise reproducible run to run.
 #include "scan_mma_kernel.cuh"
 
@@ -48,16 +55,41 @@ namespace fredec {
 
 namespace {
 
-constexpr int kNW = 8;      // warps per CTA (two per SM sub-partition)
-constexpr int kStages = 3;  // shared-memory stages of (table tile, seed records)
+constexpr int kNW = 8;         // MMA warps per CTA (two per SM sub-partition)
+constexpr int kSeedWarps = 4;  // seed warps per CTA (one per SM sub-partition)
+constexpr int kThreads = (kNW + kSeedWarps) * 32;
+// registers per thread after setmaxnreg: 128 * (2 * kRegsMma + kRegsSeed) <= 65536
+constexpr int kRegsMma = 224, kRegsSeed = 56;
+
+constexpr int kSeedGroups = 2;  // groups of 4 observations per seed warp and step at most (TI <= 32)
+
+// non-blocking: has the phase of the given parity completed?
+__device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 
 #define FREDEC_DMMA(c, a, b)                                                                  \
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"       \
         : "+d"((c)[0]), "+d"((c)[1])                                                          \
         : "d"(a), "d"(b))
 
-// Position of a CTA in its sequence of (round, tile) steps.  Three cursors walk the same
-// sequence: the loader two steps ahead, the seeder one step ahead, the MMA loop.
+// Position of a CTA in its sequence of (round, tile) steps.  The seed warps and the MMA warps
+// walk the same sequence, each with its own cursor.
 struct Cursor {
     int64_t g, g_end;  // next unit after this round / end of the CTA's range (global numbering)
     int64_t b, u;      // series and first unit (within the series) of the current round
@@ -176,198 +208,232 @@ __device__ __forceinline__ double solve_z(double YC, double YS, double CC, doubl
     return z;
 }
 
+// a9/a10 for the units of one warp after the last tile of a round: this thread holds every sum
+// of 2 * NT frequencies per unit.
 template <int H, int NOCT, int NB>
-__global__ void __launch_bounds__(kNW * 32, 1) scan_mma_kernel(MmaScanParams p)
+__device__ __forceinline__ void solve_and_store(const Tiles<H, NOCT, NB>& acc, const MmaScanParams& p, int64_t b,
+                                                int64_t unit0, int cnt, int lane)
+{
+    constexpr int R = 2 * H, NT = H / 4, NF = NB + 2;
+    const SeriesInfo info = p.info[b];
+    const int m = lane >> 2, q = lane & 3;
+    const bool last_pass = p.pass + 1 == p.n_pass;
+#pragma unroll
+    for (int o = 0; o < NOCT; ++o) {
+        if (o < cnt) {
+            const int64_t k0 = ((unit0 + o) * 8 + m) * R;  // first grid point of the run
+#pragma unroll
+            for (int t = 0; t < NT; ++t) {
+                const int h = 4 * t + q + 1;
+#pragma unroll
+                for (int sg = 0; sg < 2; ++sg) {  // sg = 0: f_c + (h - 1/2) df, 1: f_c - (h - 1/2) df
+                    const double sgn = sg == 0 ? 1.0 : -1.0;
+                    const int64_t k = sg == 0 ? k0 + H - 1 + h : k0 + H - h;
+                    double sums[NF][2];  // (cos sum, sin sum) per family
+#pragma unroll
+                    for (int f = 0; f < NF; ++f) {
+                        sums[f][0] = fma(-sgn, acc.v[o][1][f][t][1], acc.v[o][0][f][t][0]);
+                        sums[f][1] = fma(sgn, acc.v[o][0][f][t][1], acc.v[o][1][f][t][0]);
+                    }
+                    double YC = sums[0][0], YS = sums[0][1];
+                    double CC = fma(0.5, info.W, sums[NF - 1][0]), CS = sums[NF - 1][1];
+                    double Saa = 0.0, Sab = 0.0, Sbb = 0.0;
+#pragma unroll
+                    for (int j = 0; j < NB; ++j) {
+                        Saa = fma(sums[1 + j][0], sums[1 + j][0], Saa);
+                        Sab = fma(sums[1 + j][0], sums[1 + j][1], Sab);
+                        Sbb = fma(sums[1 + j][1], sums[1 + j][1], Sbb);
+                    }
+                    if (k < p.K && info.status == 0) {
+                        if (p.n_pass > 1) {  // multi-pass: carry the seven partial sums through global memory
+                            double* wsp = p.ws + (b * 7) * p.Kpad + k;
+                            if (p.pass > 0) {
+                                YC = wsp[0 * p.Kpad];
+                                YS = wsp[1 * p.Kpad];
+                                CC = wsp[2 * p.Kpad];
+                                CS = wsp[3 * p.Kpad];
+                                Saa += wsp[4 * p.Kpad];
+                                Sab += wsp[5 * p.Kpad];
+                                Sbb += wsp[6 * p.Kpad];
+                            }
+                            if (!last_pass) {
+                                if (p.pass == 0) {
+                                    wsp[0 * p.Kpad] = YC;
+                                    wsp[1 * p.Kpad] = YS;
+                                    wsp[2 * p.Kpad] = CC;
+                                    wsp[3 * p.Kpad] = CS;
+                                }
+                                wsp[4 * p.Kpad] = Saa;
+                                wsp[5 * p.Kpad] = Sab;
+                                wsp[6 * p.Kpad] = Sbb;
+                            }
+                        }
+                        if (last_pass) p.z[b * p.K + k] = solve_z(YC, YS, CC, CS, Saa, Sab, Sbb, info.W);
+                    }
+                }
+            }
+        }
+    }
+}
+
+// complex rotation (c, s) <- (c, s) * (rc, rs)
+__device__ __forceinline__ void rotate(double& c, double& s, double rc, double rs)
+{
+    const double nc = fma(c, rc, -(s * rs));
+    const double ns = fma(s, rc, c * rs);
+    c = nc;
+    s = ns;
+}
+
+template <int H, int NOCT, int NB>
+__global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
 {
     constexpr int R = 2 * H, NT = H / 4, NF = NB + 2, GROUP = NF * NT * 32, CAP = kNW * NOCT;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ __align__(8) uint64_t bar[kStages];
+    __shared__ __align__(8) uint64_t bar_tab[kMmaMaxSlots], bar_seed[kMmaMaxSlots], bar_done[kMmaMaxSlots];
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const int KS = p.TI / 4;  // groups of 4 observations per tile
+    const int KS = p.TI / 4;  // groups of 4 observations per slot
+    const int NS = p.NS;
     const size_t tab_bytes = (size_t)KS * GROUP * 8;
-    const size_t stage_bytes = tab_bytes + (size_t)p.TI * sizeof(SeedRec);
-    double2* const seeds = reinterpret_cast<double2*>(smem_raw + kStages * stage_bytes);  // [2][KS][CAP][32]
-    const size_t seed_buf = (size_t)KS * CAP * 32;
+    const size_t slot_bytes = tab_bytes + (size_t)KS * CAP * 32 * sizeof(double2);
     const int ntiles = (int)((p.G4 + KS - 1) / KS);
     const int64_t U = p.U;
 
     if (tid == 0) {
-#pragma unroll
-        for (int s = 0; s < kStages; ++s) mbar_init(&bar[s], 1);
+        for (int s = 0; s < NS; ++s) {
+            mbar_init(&bar_tab[s], 1);
+            mbar_init(&bar_seed[s], kSeedWarps);
+            mbar_init(&bar_done[s], kNW);
+        }
         mbar_fence_init();
     }
     __syncthreads();
 
     const int64_t g0 = (int64_t)blockIdx.x * p.T / p.grid, g1 = (int64_t)(blockIdx.x + 1) * p.T / p.grid;
-    Cursor ld, sd, cm;
-    ld.init(g0, g1, U, CAP);
-    sd = ld;
-    cm = ld;
-    if (!cm.valid) return;
+    Cursor c;
+    c.init(g0, g1, U, CAP);
 
-    auto issue = [&](const Cursor& c) {  // one thread: stage the tile of step c
-        const int64_t grp0 = (int64_t)c.tile * KS;
-        const int ngrp = (int)min((int64_t)KS, p.G4 - grp0);
-        const uint32_t b_tab = (uint32_t)ngrp * GROUP * 8u, b_rec = (uint32_t)ngrp * 4u * (uint32_t)sizeof(SeedRec);
-        const int st = c.step % kStages;
-        unsigned char* dst = smem_raw + st * stage_bytes;
-        mbar_expect_tx(&bar[st], b_tab + b_rec);
-        bulk_g2s(dst, p.tab + ((c.b * p.n_pass + p.pass) * p.G4 + grp0) * GROUP, b_tab, &bar[st]);
-        bulk_g2s(dst + tab_bytes, p.srec + (c.b * p.G4 + grp0) * 4, b_rec, &bar[st]);
-    };
-    auto wait_stage = [&](const Cursor& c) {
-        mbar_wait(&bar[c.step % kStages], (uint32_t)((c.step / kStages) & 1));
-    };
-    // phase A: seeds of step c into seed buffer c.step & 1
-    auto seed_tile = [&](const Cursor& c) {
-        wait_stage(c);
-        const SeedRec* recs =
-            reinterpret_cast<const SeedRec*>(smem_raw + (c.step % kStages) * stage_bytes + tab_bytes);
-        const int ngrp = (int)min((int64_t)KS, p.G4 - (int64_t)c.tile * KS);
-        double2* sb = seeds + (c.step & 1) * seed_buf + lane;
+    if (wid >= kNW) {
+        // ================= seed warps: table staging (a4) + seeds (a5) =====================
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsSeed));
+        const int pw = wid - kNW;
         const int m = lane >> 2, k = lane & 3;
-        // centre of run m of the round's first unit: f_c = f0 + (run R + H - 1/2) df   (S1)
-        const double kc = (double)((c.u * 8 + m) * R + H) - 0.5;
-        const double fc = fma(kc, p.df, p.f0);
-        for (int ks = wid; ks < ngrp; ks += kNW) {
-            const SeedRec r = recs[ks * 4 + k];
-            double cs, sn;
-            sincospi(2.0 * frac_prod(fc, r.t), &sn, &cs);
-            double2* dst = sb + (size_t)ks * CAP * 32;
-            for (int slot = 0; slot < c.n; ++slot) {
-                dst[slot * 32] = make_double2(cs, sn);
-                const double nc = fma(cs, r.cu, -(sn * r.su));
-                const double ns = fma(sn, r.cu, cs * r.su);
-                cs = nc;
-                sn = ns;
+        const SeedRec* srec = p.srec + k;
+        int slot = 0;
+        uint32_t par = 0;  // parity of the slot's current use
+        bool first_lap = true;
+        while (c.valid) {
+            const int ngrp = (int)min((int64_t)KS, p.G4 - (int64_t)c.tile * KS);
+            // this warp's records (groups pw, pw + 4) -- in flight while waiting for the slot
+            const SeedRec* rp = srec + (c.b * p.G4 + (int64_t)c.tile * KS + pw) * 4;
+            double rt[kSeedGroups], rcu[kSeedGroups], rsu[kSeedGroups], rc4[kSeedGroups], rs4[kSeedGroups];
+#pragma unroll
+            for (int j = 0; j < kSeedGroups; ++j) {
+                if (pw + kSeedWarps * j < ngrp) {
+                    const SeedRec* r = rp + kSeedWarps * j * 4;
+                    rt[j] = r->t; rcu[j] = r->cu; rsu[j] = r->su; rc4[j] = r->c4; rs4[j] = r->s4;
+                }
             }
-        }
-    };
-
-    Tiles<H, NOCT, NB> acc;
-    acc.clear();
-
-    // phase B (+ epilogue after the last tile) of step c
-    auto mma_step = [&](const Cursor& c) {
-        int off, cnt;
-        warp_share(c.n, wid, off, cnt);
-        if (cnt == 0) return;
-        wait_stage(c);
-        const double* tabs = reinterpret_cast<const double*>(smem_raw + (c.step % kStages) * stage_bytes) + lane;
-        const double2* sb = seeds + (c.step & 1) * seed_buf + (size_t)off * 32 + lane;
-        const int ngrp = (int)min((int64_t)KS, p.G4 - (int64_t)c.tile * KS);
-        if (NOCT == 1 || cnt == 1) {
-            mma_tile<1>(acc, tabs, sb, ngrp, CAP);
-        } else if (NOCT == 2 || cnt == 2) {
-            mma_tile<(NOCT >= 2 ? 2 : 1)>(acc, tabs, sb, ngrp, CAP);
-        } else if (NOCT == 3 || cnt == 3) {
-            mma_tile<(NOCT >= 3 ? 3 : 1)>(acc, tabs, sb, ngrp, CAP);
-        } else {
-            mma_tile<NOCT>(acc, tabs, sb, ngrp, CAP);
-        }
-        if (c.tile + 1 < ntiles) return;
-
-        // ---- a9/a10: this thread holds every sum of 2 * NT frequencies per unit ----------
-        const SeriesInfo info = p.info[c.b];
-        const int m = lane >> 2, q = lane & 3;
-        const bool last_pass = p.pass + 1 == p.n_pass;
+            if (!first_lap) mbar_wait(&bar_done[slot], par ^ 1u);
+            unsigned char* base = smem_raw + slot * slot_bytes;
+            if (pw == 0 && lane == 0) {
+                const uint32_t bytes = (uint32_t)ngrp * GROUP * 8u;
+                mbar_expect_tx(&bar_tab[slot], bytes);
+                bulk_g2s(base, p.tab + ((c.b * p.n_pass + p.pass) * p.G4 + (int64_t)c.tile * KS) * GROUP, bytes,
+                         &bar_tab[slot]);
+            }
+            // centre of run m of the round's first unit: f_c = f0 + (run R + H - 1/2) df   (S1)
+            const double kc = (double)((c.u * 8 + m) * R + H) - 0.5;
+            const double fc = fma(kc, p.df, p.f0);
+            double2* sb = reinterpret_cast<double2*>(base + tab_bytes) + lane;
 #pragma unroll
-        for (int o = 0; o < NOCT; ++o) {
-            if (o < cnt) {
-                const int64_t k0 = ((c.u + off + o) * 8 + m) * R;  // first grid point of the run
+            for (int j = 0; j < kSeedGroups; ++j) {
+                const int ks = pw + kSeedWarps * j;
+                if (ks < ngrp) {
+                    double cs[CAP / 4], sn[CAP / 4];
+                    sincospi(2.0 * frac_prod(fc, rt[j]), &sn[0], &cs[0]);
 #pragma unroll
-                for (int t = 0; t < NT; ++t) {
-                    const int h = 4 * t + q + 1;
+                    for (int q = 1; q < CAP / 4; ++q) {  // units 4, 8, 12: rotations by four units
+                        cs[q] = cs[q - 1];
+                        sn[q] = sn[q - 1];
+                        rotate(cs[q], sn[q], rc4[j], rs4[j]);
+                    }
+                    double2* dst = sb + (size_t)ks * CAP * 32;
 #pragma unroll
-                    for (int sg = 0; sg < 2; ++sg) {  // sg = 0: f_c + (h - 1/2) df, 1: f_c - (h - 1/2) df
-                        const double sgn = sg == 0 ? 1.0 : -1.0;
-                        const int64_t k = sg == 0 ? k0 + H - 1 + h : k0 + H - h;
-                        double sums[NF][2];  // (cos sum, sin sum) per family
+                    for (int i = 0; i < 4; ++i) {  // units 4q + i: CAP/4 independent chains
 #pragma unroll
-                        for (int f = 0; f < NF; ++f) {
-                            sums[f][0] = fma(-sgn, acc.v[o][1][f][t][1], acc.v[o][0][f][t][0]);
-                            sums[f][1] = fma(sgn, acc.v[o][0][f][t][1], acc.v[o][1][f][t][0]);
-                        }
-                        double YC = sums[0][0], YS = sums[0][1];
-                        double CC = fma(0.5, info.W, sums[NF - 1][0]), CS = sums[NF - 1][1];
-                        double Saa = 0.0, Sab = 0.0, Sbb = 0.0;
-#pragma unroll
-                        for (int j = 0; j < NB; ++j) {
-                            Saa = fma(sums[1 + j][0], sums[1 + j][0], Saa);
-                            Sab = fma(sums[1 + j][0], sums[1 + j][1], Sab);
-                            Sbb = fma(sums[1 + j][1], sums[1 + j][1], Sbb);
-                        }
-                        if (k < p.K && info.status == 0) {
-                            if (p.n_pass > 1) {  // multi-pass: carry the seven partial sums through global memory
-                                double* wsp = p.ws + (c.b * 7) * p.Kpad + k;
-                                if (p.pass > 0) {
-                                    YC = wsp[0 * p.Kpad];
-                                    YS = wsp[1 * p.Kpad];
-                                    CC = wsp[2 * p.Kpad];
-                                    CS = wsp[3 * p.Kpad];
-                                    Saa += wsp[4 * p.Kpad];
-                                    Sab += wsp[5 * p.Kpad];
-                                    Sbb += wsp[6 * p.Kpad];
-                                }
-                                if (!last_pass) {
-                                    if (p.pass == 0) {
-                                        wsp[0 * p.Kpad] = YC;
-                                        wsp[1 * p.Kpad] = YS;
-                                        wsp[2 * p.Kpad] = CC;
-                                        wsp[3 * p.Kpad] = CS;
-                                    }
-                                    wsp[4 * p.Kpad] = Saa;
-                                    wsp[5 * p.Kpad] = Sab;
-                                    wsp[6 * p.Kpad] = Sbb;
-                                }
-                            }
-                            if (last_pass) p.z[c.b * p.K + k] = solve_z(YC, YS, CC, CS, Saa, Sab, Sbb, info.W);
+                        for (int q = 0; q < CAP / 4; ++q) {
+                            dst[(4 * q + i) * 32] = make_double2(cs[q], sn[q]);
+                            if (i < 3) rotate(cs[q], sn[q], rcu[j], rsu[j]);
                         }
                     }
                 }
             }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bar_seed[slot]);
+            c.advance(ntiles, U, CAP);
+            if (++slot == NS) {
+                slot = 0;
+                par ^= 1u;
+                first_lap = false;
+            }
         }
-        acc.clear();
-    };
-
-    // ---- prologue: stage steps 0 and 1, seeds of step 0 ---------------------------------
-    if (tid == 0) {
-        issue(ld);
-        ld.advance(ntiles, U, CAP);
-        if (ld.valid) issue(ld);
-        ld.advance(ntiles, U, CAP);
     } else {
-        ld.advance(ntiles, U, CAP);
-        ld.advance(ntiles, U, CAP);
-    }
-    seed_tile(sd);
-    sd.advance(ntiles, U, CAP);
-    __syncthreads();
-
-    // ---- main loop over steps -----------------------------------------------------------
-    while (cm.valid) {
-        // stage step+2: its stage was last read in step-1, which every warp has left
-        if (tid == 0 && ld.valid) issue(ld);
-        ld.advance(ntiles, U, CAP);
-        // two warps share a sub-partition's FP64 pipe: one seeds while the other multiplies
-        if (wid < kNW / 2) {
-            if (sd.valid) seed_tile(sd);
-            mma_step(cm);
-        } else {
-            mma_step(cm);
-            if (sd.valid) seed_tile(sd);
+        // ================= MMA warps: a6 (as a contraction), a9, a10 ========================
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsMma));
+        Tiles<H, NOCT, NB> acc;
+        acc.clear();
+        int slot = 0;
+        uint32_t par = 0;
+        bool ready = false;  // the slot's barriers were seen complete one step ahead
+        while (c.valid) {
+            int off, cnt;
+            warp_share(c.n, wid, off, cnt);
+            if (!ready) {
+                mbar_wait(&bar_tab[slot], par);
+                mbar_wait(&bar_seed[slot], par);
+            }
+            // look at the next slot's barriers now; the answer is needed after this step's MMAs
+            int nslot = slot + 1;
+            uint32_t npar = par;
+            if (nslot == NS) {
+                nslot = 0;
+                npar ^= 1u;
+            }
+            ready = mbar_test(&bar_tab[nslot], npar) & mbar_test(&bar_seed[nslot], npar);
+            if (cnt > 0) {
+                const unsigned char* base = smem_raw + slot * slot_bytes;
+                const double* tabs = reinterpret_cast<const double*>(base) + lane;
+                const double2* sb = reinterpret_cast<const double2*>(base + tab_bytes) + (size_t)off * 32 + lane;
+                const int ngrp = (int)min((int64_t)KS, p.G4 - (int64_t)c.tile * KS);
+                if (NOCT == 1 || cnt == 1) {
+                    mma_tile<1>(acc, tabs, sb, ngrp, CAP);
+                } else if (NOCT == 2 || cnt == 2) {
+                    mma_tile<(NOCT >= 2 ? 2 : 1)>(acc, tabs, sb, ngrp, CAP);
+                } else if (NOCT == 3 || cnt == 3) {
+                    mma_tile<(NOCT >= 3 ? 3 : 1)>(acc, tabs, sb, ngrp, CAP);
+                } else {
+                    mma_tile<NOCT>(acc, tabs, sb, ngrp, CAP);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bar_done[slot]);
+            if (c.tile + 1 == ntiles && cnt > 0) {
+                solve_and_store<H, NOCT, NB>(acc, p, c.b, c.u + off, cnt, lane);
+                acc.clear();
+            }
+            c.advance(ntiles, U, CAP);
+            slot = nslot;
+            par = npar;
         }
-        sd.advance(ntiles, U, CAP);
-        cm.advance(ntiles, U, CAP);
-        __syncthreads();
     }
 }
 
 template <int H, int NOCT, int NB>
 cudaError_t launch_one(const MmaScanParams& p, cudaStream_t stream)
 {
-    const size_t smem = mma_scan_smem_bytes(NB, p.TI);
+    const size_t smem = (size_t)p.NS * mma_scan_slot_bytes(NB, p.TI);
     static size_t attr_smem = 0;
     if (smem > attr_smem) {
         cudaError_t e = cudaFuncSetAttribute(scan_mma_kernel<H, NOCT, NB>,
@@ -375,7 +441,8 @@ cudaError_t launch_one(const MmaScanParams& p, cudaStream_t stream)
         if (e != cudaSuccess) return e;
         attr_smem = smem;
     }
-    scan_mma_kernel<H, NOCT, NB><<<p.grid, kNW * 32, smem, stream>>>(p);
+    if (p.NS < 2 || p.NS > kMmaMaxSlots || p.TI < 4 || p.TI % 4 || p.TI > 16 * kSeedGroups) return cudaErrorInvalidValue;
+    scan_mma_kernel<H, NOCT, NB><<<p.grid, kThreads, smem, stream>>>(p);
     return cudaGetLastError();
 }
 
@@ -383,7 +450,7 @@ cudaError_t launch_one(const MmaScanParams& p, cudaStream_t stream)
 
 // (H, NOCT) per NB: NOCT * (2 + NB) * H accumulator doubles per thread
 #define FREDEC_MMA_CONFIGS(X) \
-    X(8, 2, 0) X(8, 2, 1) X(8, 2, 2) X(8, 2, 3) X(8, 1, 4) X(8, 1, 5) X(8, 1, 6) X(8, 1, 7) X(8, 1, 8) X(8, 1, 9)
+    X(16, 2, 0) X(16, 1, 1) X(16, 1, 2) X(8, 2, 3) X(8, 1, 4) X(8, 1, 5) X(8, 1, 6) X(8, 1, 7) X(8, 1, 8) X(8, 1, 9)
 
 MmaScanConfig mma_scan_config(int NB)
 {
@@ -394,12 +461,10 @@ MmaScanConfig mma_scan_config(int NB)
     return MmaScanConfig{0, 0, 0};
 }
 
-size_t mma_scan_smem_bytes(int NB, int TI)
+size_t mma_scan_slot_bytes(int NB, int TI)
 {
     const MmaScanConfig c = mma_scan_config(NB);
-    const size_t stage = (size_t)(TI / 4) * mma_group_doubles(c.H, NB) * 8 + (size_t)TI * sizeof(SeedRec);
-    const size_t seeds = 2 * (size_t)(TI / 4) * (c.NW * c.NOCT) * 32 * 16;
-    return kStages * stage + seeds;
+    return (size_t)(TI / 4) * (mma_group_doubles(c.H, NB) * 8 + (size_t)(c.NW * c.NOCT) * 32 * 16);
 }
 
 cudaError_t launch_mma_scan(int NB, const MmaScanParams& p, cudaStream_t stream)

@@ -22,9 +22,10 @@ __host__ __device__ constexpr int mma_nt(int H) { return H / 4; }
 __host__ __device__ constexpr int mma_nf(int NB) { return NB + 2; }
 __host__ __device__ constexpr int mma_group_doubles(int H, int NB) { return mma_nf(NB) * mma_nt(H) * 32; }
 
-// Per-observation seed record: t', (cos, sin) of the rotation by one unit (8 runs = 8R grid steps).
-struct __align__(32) SeedRec {
-    double t, cu, su, pad;
+// Per-observation seed record: t', (cos, sin) of the rotation by one unit (8 runs = 8R grid
+// steps) and by four units.
+struct __align__(16) SeedRec {
+    double t, cu, su, c4, s4, pad;
 };
 
 struct MmaScanParams {
@@ -39,18 +40,20 @@ struct MmaScanParams {
     int64_t T;   // total units = B * U
     double f0, df;
     int n_pass, pass;
-    int TI;    // observations per shared-memory tile (multiple of 4 * warps per CTA)
+    int TI;    // observations per shared-memory slot (multiple of 4)
+    int NS;    // slots of the (table tile, seeds) ring in shared memory
     int grid;  // CTAs (persistent; each owns a contiguous range of units)
 };
 
 struct MmaScanConfig {
-    int H, NOCT, NW;  // half run length, units per warp and round, warps per CTA
+    int H, NOCT, NW;  // half run length, units per MMA warp and round, MMA warps per CTA
 };
 
 // The (H, NOCT) the library is built with for NB base functions per pass (NB <= kMmaMaxNB).
 constexpr int kMmaMaxNB = 9;
 MmaScanConfig mma_scan_config(int NB);
-size_t mma_scan_smem_bytes(int NB, int TI);
+size_t mma_scan_slot_bytes(int NB, int TI);  // one ring slot; the kernel needs NS of them
+constexpr int kMmaMaxSlots = 8;
 cudaError_t launch_mma_scan(int NB, const MmaScanParams& p, cudaStream_t stream);
 
 }  // namespace fredec
