@@ -4,14 +4,15 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path (validate/centre,
-base orthogonalisation, packing, scan with fused solve, peak extraction) over the
+base orthogonalisation, per-observation table, scan with fused solve, peak extraction) over the
 survey-scale workload (config 4: N = 10 000 observations x K = 2 000 000 grid frequencies,
 base = offset + trend), one `fredec_scan_topk` call through the C-ABI binding.
 
   value     (frequency x observation) pairs per second, whole job, inputs resident in HBM
   e2e       the same with HOST (pinned) buffers: H2D of t, x, w, base and D2H of z and the
             peak indices inside the timed region
-  roofline  the scan kernel against the FP64 FMA pipe (bound "alu")
+  roofline  the scan kernel against the FP64 FMA rate of the chip (bound "alu"; the kernel issues
+            its FMAs as FP64 MMA instructions, which run at the same 64 FMA/clk/SM)
   cpu_baseline  the CPU oracle, as it stands, on a bounded sample of the same workload
 
 N > 1 (torchrun): weak scaling, rank r scans grid points [r K, (r+1) K) of a grid of N K
@@ -40,17 +41,19 @@ WORKLOAD = "config4 survey: N=10000 obs x K=2000000 freqs, d=2 (offset+trend), t
 FP64_LANES_PER_SM = 64
 L2_FLUSH_BYTES = 256 << 20
 ORACLE_SAMPLE_K = 20_000          # grid points of config 4 the CPU legs time per step
-# dram__bytes_read.sum + dram__bytes_write.sum of one scan_kernel launch on config 4, from the
-# `ncu --set full` capture summarised in profiles/r1_scan_kernel_ncu.md (849 920 B read, 0 B written:
-# the 16 MB periodogram is still in L2 when the kernel ends).  Algorithmic bytes: 0.8 MB + 16 MB.
-SCAN_DRAM_TRAFFIC_BYTES = 849_920
+# dram__bytes_read.sum + dram__bytes_write.sum of one scan_mma_kernel launch on config 4, from the
+# `ncu --set full` capture summarised in profiles/r1_scan_mma_kernel_ncu.md (read only: the 16 MB
+# periodogram is still in L2 when the kernel ends).  Algorithmic bytes: 10.6 MB table + 16 MB z.
+SCAN_DRAM_TRAFFIC_BYTES = 11_000_000
 
 
 def flops_per_pair(d: int) -> int:
-    """Algorithmic FP64 flops per (frequency, observation) pair, for the
-    two-term recurrence the kernel executes: accumulate (4+2d) FMA + 1 MUL = 9+4d, advance
-    2 FMA = 4.  (The rotation form would be 15+4d; flops that are not executed are not credited.)"""
-    return 13 + 4 * d
+    """FP64 flops per (frequency, observation) pair that the scan kernel executes for the sums of
+    SURVEY.md 8(a) row a6: one FMA per (pair, sum), 4+2d sums (YC, YS, CC, CS, A_j, B_j), all in
+    FP64 MMA instructions.  The product form has no per-pair MUL and no
+    per-pair recurrence, so SURVEY 8(d)'s 15+4d (rotation form) is not what runs; flops that are
+    not executed are not credited.  Seeds, reductions and the epilogue are overhead, not counted."""
+    return 2 * (4 + 2 * d)
 
 
 class ClockSampler:
@@ -309,7 +312,7 @@ def main_ours(args):
         "kernel_ms": {"prep": kern["prep_ms"] / args.steps, "scan": scan_ms, "topk": kern["topk_ms"] / args.steps},
         "fraction_of_fp64_peak": achieved / peak_nominal,
         "fraction_of_fp64_peak_rotation_form_equivalent": achieved / peak_nominal * (15 + 4 * wl.d) / F,
-        "roofline": {"bound": "alu", "kernel": "scan_kernel", "achieved": achieved, "peak": peak_nominal,
+        "roofline": {"bound": "alu", "kernel": "scan_mma_kernel", "achieved": achieved, "peak": peak_nominal,
                      "unit": "TFLOP/s", "frac": achieved / peak_nominal, "traffic": SCAN_DRAM_TRAFFIC_BYTES,
                      "flops_per_pair": F, "peak_source": f"nominal: {sm_count} SMs x {FP64_LANES_PER_SM} FP64 FMA "
                      "lanes x 2 x 1.965 GHz (DESIGN.md section 6)",

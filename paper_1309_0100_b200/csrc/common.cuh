@@ -6,23 +6,6 @@
 
 namespace fredec {
 
-// ---------------------------------------------------------------------------------------
-// Packed observation record (written by the prep kernel, staged tile by tile into shared
-// memory by the scan kernel).  One record = kHdr header doubles + NBP base values, where
-// NBP = NB rounded up to even so that every record is a whole number of 16-byte words
-// (cp.async.bulk and LDS.128 alignment).
-//
-//   [0] t'      centred time t_i - (t_min + t_max)/2           (S10: z is origin-invariant)
-//   [1] 2 cos of 2 pi frac(df * t')           : coefficient of the two-term recurrence
-//   [2] cos, [3] sin of 2 pi frac(df * t')      : one grid step for this observation
-//   [4] cos, [5] sin of 2 pi frac(R * df * t')  : one RUN step (R grid steps)
-//   [6] w_i     weight                                          (0 in passes > 0)
-//   [7] y_i     w_i * (x_i - base fit)                          (0 in passes > 0)
-//   [8..]       p_ji = w_i * psi_j(t_i), psi = orthonormalised base functions of this pass
-// ---------------------------------------------------------------------------------------
-constexpr int kHdr = 8;
-__host__ __device__ constexpr int rec_stride(int nb) { return kHdr + ((nb + 1) & ~1); }
-
 // Per-series scalars produced by the prep kernel.
 struct SeriesInfo {
     double W;          // <1> = sum w

@@ -10,7 +10,6 @@
 #include "fredec.h"
 #include "peak_kernel.cuh"
 #include "prep_kernel.cuh"
-#include "scan_kernel.cuh"
 #include "scan_mma_kernel.cuh"
 #include "topk_kernel.cuh"
 
@@ -75,7 +74,7 @@ struct State {
     cudaStream_t stream = nullptr;
     cudaEvent_t ev[kNumEvents] = {};
     DevBuf in_t, in_x, in_w, in_base, in_z, out_z, out_idx, out_chi2;
-    DevBuf rec, tab, srec, psi, xt, info, ws, part_z, part_i, count, sink;
+    DevBuf tab, srec, psi, xt, info, ws, red, part_z, part_i, count, sink;
     HostBuf h_info, h_count;
     int last_cuda = 0;
     double timing[4] = {0, 0, 0, 0};
@@ -154,44 +153,6 @@ int stage_out(T* dst, size_t count, DevBuf& buf, T** out, T** host_dst)
     return FREDEC_OK;
 }
 
-struct ScanPlan {
-    int R, NB, n_pass, FW, S, TI;
-};
-
-ScanPlan plan_scan(int64_t B, int64_t N, int d, int64_t K)
-{
-    ScanPlan pl;
-    if (d <= 3) {
-#ifdef FREDEC_PLAN_R_SMALL
-        pl.R = FREDEC_PLAN_R_SMALL; pl.NB = d; pl.n_pass = 1;
-#else
-        pl.R = 8; pl.NB = d; pl.n_pass = 1;
-#endif
-    } else if (d <= 9) {
-        pl.R = 4; pl.NB = d; pl.n_pass = 1;
-    } else {
-        pl.R = 4; pl.NB = 8; pl.n_pass = (d + 7) / 8;
-    }
-    const int64_t runs = (K + pl.R - 1) / pl.R;
-    const int64_t fwarps = (runs + 31) / 32 * B;   // warps if every run had its own lane once
-    const int64_t target = (int64_t)g.sm_count * 8;
-    const int max_warps = scan_max_warps();
-    int S = 1;
-    while (S * 2 <= max_warps && fwarps * (S * 2) <= target && N / (S * 2) >= 16) S *= 2;
-    int FW = 1;
-    while (FW < 4 && FW * 2 * S <= max_warps && fwarps / (FW * 2) >= 2 * (int64_t)g.sm_count) FW *= 2;
-    pl.S = S;
-    pl.FW = FW;
-#ifndef FREDEC_PLAN_SEED_ELEMS
-#define FREDEC_PLAN_SEED_ELEMS 4096
-#endif
-    int TI = FREDEC_PLAN_SEED_ELEMS / (FW * 32);   // seeds: J x (TI+1) x 16 B ~ 64 KB per CTA
-    if (TI > 128) TI = 128;
-    if (N < TI) TI = (int)((N + S - 1) / S * S);
-    pl.TI = TI;
-    return pl;
-}
-
 int check_series_args(const double* t, const double* x, const double* w, int64_t B, int64_t N,
                       const double* base_funcs, int32_t d)
 {
@@ -262,9 +223,8 @@ int enqueue_series_mma(Call& c, const double* dt, const double* dx, const double
     PrepParams pp;
     pp.t = dt; pp.x = dx; pp.w = dw; pp.base = dbase;
     pp.psi = g.psi.as<double>(); pp.xt = g.xt.as<double>();
-    pp.rec = nullptr;
     pp.info = g.info.as<SeriesInfo>();
-    pp.N = N; pp.d = d; pp.NB = NB; pp.n_pass = n_pass; pp.R = R; pp.df = df;
+    pp.N = N; pp.d = d;
     CK(cudaEventRecord(g.ev[1], st));
     CK(launch_prep(pp, B, st));
     TableParams tp;
@@ -305,6 +265,8 @@ int enqueue_series_mma(Call& c, const double* dt, const double* dx, const double
         CK(g.ws.reserve((size_t)B * 7 * sp.Kpad * 8));
         sp.ws = g.ws.as<double>();
     }
+    CK(g.red.reserve((size_t)sp.grid * cfg.NW * mma_red_doubles(NB) * 8));
+    sp.red = g.red.as<double>();
     for (int pass = 0; pass < n_pass; ++pass) {
         sp.pass = pass;
         CK(launch_mma_scan(NB, sp, st));
@@ -331,58 +293,22 @@ int enqueue_series(Call& c, const double* t, const double* x, const double* w, i
     if ((rc = stage_in(w, BN, g.in_w, &dw))) return rc;
     if ((rc = stage_in(base_funcs, BN * d, g.in_base, &dbase))) return rc;
 
-    static const bool use_old = std::getenv("FREDEC_SCAN_OLD") != nullptr;
-    if (with_scan && !use_old) return enqueue_series_mma(c, dt, dx, dw, dbase, B, N, d, f0, df, K, z_out);
+    if (with_scan) return enqueue_series_mma(c, dt, dx, dw, dbase, B, N, d, f0, df, K, z_out);
 
-    ScanPlan pl = plan_scan(B, N, d, with_scan ? K : 1);
-    const int RS = rec_stride(pl.NB);
+    // base fit only (chi2_base): the prep kernel alone
     CK(g.psi.reserve(BN * (size_t)(d > 0 ? d : 1) * 8));
     CK(g.xt.reserve(BN * 8));
     CK(g.info.reserve((size_t)B * sizeof(SeriesInfo)));
     CK(g.h_info.reserve((size_t)B * sizeof(SeriesInfo)));
-    if (with_scan) CK(g.rec.reserve(BN * pl.n_pass * RS * 8));
-
     PrepParams pp;
     pp.t = dt; pp.x = dx; pp.w = dw; pp.base = dbase;
     pp.psi = g.psi.as<double>(); pp.xt = g.xt.as<double>();
-    pp.rec = with_scan ? g.rec.as<double>() : nullptr;
     pp.info = g.info.as<SeriesInfo>();
-    pp.N = N; pp.d = d; pp.NB = pl.NB; pp.n_pass = pl.n_pass; pp.R = pl.R; pp.df = with_scan ? df : 1.0;
+    pp.N = N; pp.d = d;
     CK(cudaEventRecord(g.ev[1], st));
     CK(launch_prep(pp, B, st));
     g.launches += 1;
     CK(cudaEventRecord(g.ev[2], st));
-
-    if (with_scan) {
-        c.z_count = (size_t)B * K;
-        if (z_out == nullptr) {
-            CK(g.out_z.reserve(c.z_count * 8));
-            c.dz = g.out_z.as<double>();
-            c.hz = nullptr;
-        } else if ((rc = stage_out(z_out, c.z_count, g.out_z, &c.dz, &c.hz))) {
-            return rc;
-        }
-        ScanParams sp;
-        sp.rec = g.rec.as<double>();
-        sp.info = g.info.as<SeriesInfo>();
-        sp.z = c.dz;
-        sp.N = N; sp.K = K;
-        const int64_t runs = (K + pl.R - 1) / pl.R;
-        sp.Kpad = runs * pl.R;
-        sp.f0 = f0; sp.df = df;
-        sp.n_pass = pl.n_pass;
-        sp.FW = pl.FW; sp.S = pl.S; sp.TI = pl.TI;
-        sp.ws = nullptr;
-        if (pl.n_pass > 1) {
-            CK(g.ws.reserve((size_t)B * 7 * sp.Kpad * 8));
-            sp.ws = g.ws.as<double>();
-        }
-        for (int pass = 0; pass < pl.n_pass; ++pass) {
-            sp.pass = pass;
-            CK(launch_scan(pl.R, pl.NB, sp, B, st));
-            g.launches += 1;
-        }
-    }
     CK(cudaEventRecord(g.ev[3], st));
     c.B = B;
     c.has_series = true;
@@ -606,8 +532,8 @@ int fredec_fp64_peak(int64_t iters, double* tflops_out, double* ms_out)
 
 int fredec_shutdown(void)
 {
-    DevBuf* bufs[] = {&g.in_t, &g.in_x, &g.in_w, &g.in_base, &g.in_z, &g.out_z, &g.out_idx, &g.out_chi2, &g.rec, &g.tab, &g.srec,
-                      &g.psi,  &g.xt,   &g.info, &g.ws,      &g.part_z, &g.part_i, &g.count, &g.sink};
+    DevBuf* bufs[] = {&g.in_t, &g.in_x, &g.in_w, &g.in_base, &g.in_z, &g.out_z, &g.out_idx, &g.out_chi2, &g.tab, &g.srec,
+                      &g.psi,  &g.xt,   &g.info, &g.ws, &g.red,     &g.part_z, &g.part_i, &g.count, &g.sink};
     for (DevBuf* b : bufs) b->release();
     g.h_info.release();
     g.h_count.release();

@@ -1,5 +1,6 @@
 // prep_kernel.cu -- steps a1-a3 of the scan: validate, centre, orthogonalise the base
-// model, pack per-observation records.  Once per scan, one CTA per series.
+// model (prep_kernel, one CTA per series), per-observation table and seed records
+// (table_kernel).  Once per scan.
 //
 // Generalises the normalisations of PAPER.md:193-197 (eq. 18: <1> = 1, <x> = 0, ...) to an
 // arbitrary linear base model: the base functions are replaced by functions psi_j that are
@@ -132,38 +133,9 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p)
         info->status = status;
         info->pad = 0;
     }
-    if (status != 0 || p.rec == nullptr) return;
-
-    // ---- a3: step constants and packing ---------------------------------------------------
-    const int RS = rec_stride(p.NB);
-    const int NBP = RS - kHdr;
-    const double dfR = p.df * (double)p.R;  // exact: R is a power of two
-    for (int pass = 0; pass < p.n_pass; ++pass) {
-        double* rec = p.rec + ((b * p.n_pass + pass) * N) * RS;
-        for (int64_t i = threadIdx.x; i < N; i += kPrepThreads) {
-            double* r = rec + i * RS;
-            const double tc = t[i] - t_mid;
-            double c1, s1, cR, sR;
-            sincospi(2.0 * frac_prod(p.df, tc), &s1, &c1);
-            sincospi(2.0 * frac_prod(dfR, tc), &sR, &cR);
-            const double wi = w[i];
-            r[0] = tc;
-            r[1] = 2.0 * c1;
-            r[2] = c1;
-            r[3] = s1;
-            r[4] = cR;
-            r[5] = sR;
-            r[6] = pass == 0 ? wi : 0.0;
-            r[7] = pass == 0 ? wi * xt[i] : 0.0;
-            for (int m = 0; m < NBP; ++m) {
-                const int j = pass * p.NB + m;
-                r[kHdr + m] = (m < p.NB && j < d) ? wi * psi[(int64_t)j * N + i] : 0.0;
-            }
-        }
-    }
 }
 
-// ---- a3 for the MMA scan: per-observation table and seed records --------------------------
+// ---- a3: per-observation table and seed records --------------------------
 // One thread per observation (padded to whole groups of 4 with zero multipliers).  Layout:
 // scan_mma_kernel.cuh.
 constexpr int kTableThreads = 128;
@@ -184,8 +156,7 @@ __global__ void __launch_bounds__(kTableThreads) table_kernel(TableParams p)
         SeedRec r;
         r.t = tc;
         sincospi(2.0 * frac_prod(p.df * (double)(16 * H), tc), &r.su, &r.cu);  // one unit = 8 runs of 2H steps
-        sincospi(2.0 * frac_prod(p.df * (double)(64 * H), tc), &r.s4, &r.c4);  // four units
-        r.pad = 0.0;
+        r.tcu = 2.0 * r.cu;
         p.srec[b * p.G4 * 4 + i] = r;
     }
     double* grp = p.tab + ((b * p.n_pass + pass) * p.G4 + i / 4) * mma_group_doubles(H, p.NB);

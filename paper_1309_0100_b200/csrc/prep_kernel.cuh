@@ -12,17 +12,12 @@ struct PrepParams {
     const double* base;  // [B][d][N] or nullptr when d == 0
     double* psi;         // workspace [B][d][N]
     double* xt;          // workspace [B][N]
-    double* rec;         // out [B][n_pass][N][rec_stride(NB)], or nullptr: scalars only
     SeriesInfo* info;    // out [B]
     int64_t N;
     int d;
-    int NB;      // base functions per pass
-    int n_pass;  // ceil(d / NB), >= 1
-    int R;       // grid steps per run (power of two)
-    double df;
 };
 
-// a3 for the MMA scan (scan_mma_kernel.cuh): table + seed records from the prep kernel's psi, x~
+// a3 (layouts: scan_mma_kernel.cuh): table + seed records from the prep kernel's psi, x~
 struct TableParams {
     const double* t;         // [B][N]
     const double* w;         // [B][N]

@@ -39,12 +39,17 @@
 //           (mbarrier "done"); one lane stages the table tile global -> shared by 1-D TMA
 //           (cp.async.bulk, mbarrier "tab"); then a5: seeds e^{i phi} for every (run of the
 //           round, observation of the tile) in A-fragment order -- one exact evaluation
-//           (range-reduced phase, sincospi) at the round's first unit, rotations by 4 units and
-//           by 1 unit for the others (four independent chains) -- and arrive on mbarrier "seed".
+//           (range-reduced phase, table + short polynomial) at the round's first unit, one
+//           rotation to the second, then the two-term recurrence e_{u+1} = 2 cos(theta) e_u -
+//           e_{u-1} along the units -- and arrive on mbarrier "seed".
 //   MMA warps (8, two per sub-partition)  wait for "tab" and "seed"; per 4 observations:
 //           A fragments (seeds; double-angle seeds by 4 flops), B fragments (table),
 //           2 * NF * NT MMAs per unit; arrive on "done".  After the last tile of a round the
 //           thread that holds all sums of a frequency solves (a9) and stores z (a10).
+//
+// Rounds hold a power of two of units.  A round of fewer units than MMA warps (the tail of a
+// CTA's range, or a short grid) splits the observations between the warps that share a unit
+// (a8); their partial sums are added in fixed order through a per-CTA scratch in global memory.
 //
 // The seed warps run up to NS steps ahead of the MMA warps, so the latency of the seed chains
 // (which share the FP64 pipe with the MMAs) is off the MMA warps' critical path.
@@ -59,7 +64,7 @@ constexpr int kNW = 8;         // MMA warps per CTA (two per SM sub-partition)
 constexpr int kSeedWarps = 4;  // seed warps per CTA (one per SM sub-partition)
 constexpr int kThreads = (kNW + kSeedWarps) * 32;
 // registers per thread after setmaxnreg: 128 * (2 * kRegsMma + kRegsSeed) <= 65536
-constexpr int kRegsMma = 224, kRegsSeed = 56;
+constexpr int kRegsMma = 216, kRegsSeed = 72;
 
 constexpr int kSeedGroups = 2;  // groups of 4 observations per seed warp and step at most (TI <= 32)
 
@@ -105,6 +110,7 @@ struct Cursor {
         int64_t m = U - u;
         if (g_end - g < m) m = g_end - g;
         n = m < cap ? (int)m : cap;
+        n = 1 << (31 - __clz(n));  // a power of two: rounds smaller than kNW split the observations
     }
     __device__ __forceinline__ void init(int64_t g0, int64_t g1, int64_t U, int cap)
     {
@@ -115,6 +121,12 @@ struct Cursor {
         valid = g < g_end;
         b = u = 0;
         n = 0;
+        if (valid) set_round(U, cap);
+    }
+    __device__ __forceinline__ void next_round(int64_t U, int cap)
+    {
+        g += n;
+        valid = g < g_end;
         if (valid) set_round(U, cap);
     }
     __device__ __forceinline__ void advance(int ntiles, int64_t U, int cap)
@@ -129,12 +141,29 @@ struct Cursor {
     }
 };
 
-// units of the round owned by warp w: cnt units starting at slot off
-__device__ __forceinline__ void warp_share(int n, int w, int& off, int& cnt)
+// Role of MMA warp w in a round of n units (n a power of two <= kNW * NOCT):
+//   n >= kNW  the warp owns cnt = n / kNW units starting at slot off, all observations (S = 1)
+//   n <  kNW  S = kNW / n warps share the unit in slot off; the warp takes the groups of 4
+//             observations with (group within the ring slot) % S == sp  (a8: observation split;
+//             the partial sums are added in fixed order before the solve)
+struct WarpRole {
+    int off, cnt, S, sp;
+};
+__device__ __forceinline__ WarpRole warp_role(int n, int w)
 {
-    const int q = n / kNW, r = n - q * kNW;
-    cnt = q + (w < r ? 1 : 0);
-    off = w * q + (w < r ? w : r);
+    WarpRole r;
+    if (n >= kNW) {
+        r.cnt = n / kNW;
+        r.off = w * r.cnt;
+        r.S = 1;
+        r.sp = 0;
+    } else {
+        r.cnt = 1;
+        r.S = kNW / n;
+        r.off = w / r.S;
+        r.sp = w % r.S;
+    }
+    return r;
 }
 
 template <int H, int NOCT, int NB>
@@ -154,39 +183,86 @@ struct Tiles {
     }
 };
 
-// phase B for one tile: CNT = units this warp owns in the round
+// Ring position of a warp: the slot it is at, the parity of the slot's current use, and whether
+// the slot's "tab" and "seed" barriers were already seen complete (looked at one slot ahead).
+struct RingPos {
+    int slot;
+    uint32_t par;
+    bool ready;
+};
+
+// a6 for one round: all tiles of the series, CNT = units this warp owns in the round.  One flat
+// loop over the groups of 4 observations; the ring slot changes every KS groups without leaving
+// the loop, so the MMA stream continues across slots.
 template <int CNT, int H, int NOCT, int NB>
-__device__ __forceinline__ void mma_tile(Tiles<H, NOCT, NB>& acc, const double* tabs, const double2* sb, int ngrp,
-                                         int cap)
+__device__ __forceinline__ void round_mma(Tiles<H, NOCT, NB>& acc, RingPos& rp, const unsigned char* smem,
+                                          size_t slot_bytes, size_t tab_bytes, int NS, int KS, int64_t G4,
+                                          WarpRole role, int lane, uint64_t* bar_tab, uint64_t* bar_seed,
+                                          uint64_t* bar_done)
 {
-    constexpr int NT = H / 4, NF = NB + 2, GROUP = NF * NT * 32;
+    constexpr int NT = H / 4, NF = NB + 2, GROUP = NF * NT * 32, CAP = kNW * NOCT;
+    const double* tk = nullptr;
+    const double2* sk = nullptr;
+    int ksl = 0;
+    int nslot = 0;
+    uint32_t npar = 0;
 #pragma unroll 1
-    for (int ks = 0; ks < ngrp; ++ks) {
-        double2 a[CNT];
-        double c2[CNT], s2[CNT];
-#pragma unroll
-        for (int o = 0; o < CNT; ++o) {
-            a[o] = sb[((size_t)ks * cap + o) * 32];
-            c2[o] = fma(a[o].x, a[o].x, -(a[o].y * a[o].y));  // cos 2 phi
-            s2[o] = (a[o].x + a[o].x) * a[o].y;              // sin 2 phi
+    for (int64_t g = 0; g < G4; ++g) {
+        if (ksl == 0) {  // enter the slot
+            if (!rp.ready) {
+                mbar_wait(&bar_tab[rp.slot], rp.par);
+                mbar_wait(&bar_seed[rp.slot], rp.par);
+            }
+            const unsigned char* base = smem + rp.slot * slot_bytes;
+            tk = reinterpret_cast<const double*>(base) + lane;
+            sk = reinterpret_cast<const double2*>(base + tab_bytes) + (size_t)role.off * 32 + lane;
+            nslot = rp.slot + 1;
+            npar = rp.par;
+            if (nslot == NS) {
+                nslot = 0;
+                npar ^= 1u;
+            }
+            rp.ready = false;
         }
-        const double* tk = tabs + (size_t)ks * GROUP;
+        if (CNT > 0 && (ksl & (role.S - 1)) == role.sp) {
+            double2 a[CNT > 0 ? CNT : 1];
+            double c2[CNT > 0 ? CNT : 1], s2[CNT > 0 ? CNT : 1];
 #pragma unroll
-        for (int f = 0; f < NF; ++f) {
+            for (int o = 0; o < CNT; ++o) {
+                a[o] = sk[o * 32];
+                c2[o] = fma(a[o].x, a[o].x, -(a[o].y * a[o].y));  // cos 2 phi
+                s2[o] = (a[o].x + a[o].x) * a[o].y;              // sin 2 phi
+            }
 #pragma unroll
-            for (int t = 0; t < NT; ++t) {
-                const double bf = tk[(f * NT + t) * 32];
+            for (int f = 0; f < NF; ++f) {
 #pragma unroll
-                for (int o = 0; o < CNT; ++o) {
-                    if (f < NF - 1) {
-                        FREDEC_DMMA(acc.v[o][0][f][t], a[o].x, bf);
-                        FREDEC_DMMA(acc.v[o][1][f][t], a[o].y, bf);
-                    } else {
-                        FREDEC_DMMA(acc.v[o][0][f][t], c2[o], bf);
-                        FREDEC_DMMA(acc.v[o][1][f][t], s2[o], bf);
+                for (int t = 0; t < NT; ++t) {
+                    const double bf = tk[(f * NT + t) * 32];
+#pragma unroll
+                    for (int o = 0; o < CNT; ++o) {
+                        if (f < NF - 1) {
+                            FREDEC_DMMA(acc.v[o][0][f][t], a[o].x, bf);
+                            FREDEC_DMMA(acc.v[o][1][f][t], a[o].y, bf);
+                        } else {
+                            FREDEC_DMMA(acc.v[o][0][f][t], c2[o], bf);
+                            FREDEC_DMMA(acc.v[o][1][f][t], s2[o], bf);
+                        }
                     }
                 }
             }
+        }
+        tk += GROUP;
+        sk += CAP * 32;
+        ++ksl;
+        if (ksl == KS - 1 || KS == 1) {  // one group before the end: is the next slot there already?
+            rp.ready = mbar_test(&bar_tab[nslot], npar) & mbar_test(&bar_seed[nslot], npar);
+        }
+        if (ksl == KS || g + 1 == G4) {  // leave the slot
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bar_done[rp.slot]);
+            rp.slot = nslot;
+            rp.par = npar;
+            ksl = 0;
         }
     }
 }
@@ -276,6 +352,28 @@ __device__ __forceinline__ void solve_and_store(const Tiles<H, NOCT, NB>& acc, c
     }
 }
 
+// (cos, sin)(2 pi x) for |x| <= 1/2 (+ rounding): x = j/64 + r with |r| <= 1/128, the j part
+// from a 64-entry table in shared memory, the r part by Taylor polynomials in y = 2 pi r
+// (|y| <= 0.0491: truncation errors y^10/10! < 3e-20 and y^9/9! < 5e-18), combined by one
+// complex rotation.  About 20 FP64 instructions instead of ~45 for sincospi.
+__device__ __forceinline__ void sincos_turns(double x, const double2* trig64, double& c, double& s)
+{
+    const double jd = rint(x * 64.0);
+    const double r = fma(jd, -0.015625, x);  // exact
+    const double2 tj = trig64[(int)jd & 63];
+    const double y = r * 6.283185307179586477;
+    const double y2 = y * y;
+    double pc = fma(y2, 1.0 / 40320.0, -1.0 / 720.0);
+    pc = fma(pc, y2, 1.0 / 24.0);
+    pc = fma(pc, y2, -0.5);
+    pc = fma(pc, y2, 1.0);  // cos y
+    double ps = fma(y2, -1.0 / 5040.0, 1.0 / 120.0);
+    ps = fma(ps, y2, -1.0 / 6.0);
+    ps = fma(ps * y2, y, y);  // sin y
+    c = fma(tj.x, pc, -(tj.y * ps));
+    s = fma(tj.y, pc, tj.x * ps);
+}
+
 // complex rotation (c, s) <- (c, s) * (rc, rs)
 __device__ __forceinline__ void rotate(double& c, double& s, double rc, double rs)
 {
@@ -291,6 +389,7 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
     constexpr int R = 2 * H, NT = H / 4, NF = NB + 2, GROUP = NF * NT * 32, CAP = kNW * NOCT;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     __shared__ __align__(8) uint64_t bar_tab[kMmaMaxSlots], bar_seed[kMmaMaxSlots], bar_done[kMmaMaxSlots];
+    __shared__ double2 trig64[64];  // (cos, sin)(2 pi j / 64)
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int KS = p.TI / 4;  // groups of 4 observations per slot
@@ -300,6 +399,11 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
     const int ntiles = (int)((p.G4 + KS - 1) / KS);
     const int64_t U = p.U;
 
+    if (tid >= 64 && tid < 128) {
+        double sj, cj;
+        sincospi((double)(tid - 64) * 0.03125, &sj, &cj);
+        trig64[tid - 64] = make_double2(cj, sj);
+    }
     if (tid == 0) {
         for (int s = 0; s < NS; ++s) {
             mbar_init(&bar_tab[s], 1);
@@ -323,56 +427,70 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
         int slot = 0;
         uint32_t par = 0;  // parity of the slot's current use
         bool first_lap = true;
-        while (c.valid) {
-            const int ngrp = (int)min((int64_t)KS, p.G4 - (int64_t)c.tile * KS);
-            // this warp's records (groups pw, pw + 4) -- in flight while waiting for the slot
-            const SeedRec* rp = srec + (c.b * p.G4 + (int64_t)c.tile * KS + pw) * 4;
-            double rt[kSeedGroups], rcu[kSeedGroups], rsu[kSeedGroups], rc4[kSeedGroups], rs4[kSeedGroups];
+        // this warp's records (groups pw, pw + 4 of the slot) are fetched one step ahead
+        double nt_[kSeedGroups], ncu[kSeedGroups], nsu[kSeedGroups], ntc[kSeedGroups];
+        auto fetch = [&](const Cursor& cc) {
+            const int ng = (int)min((int64_t)KS, p.G4 - (int64_t)cc.tile * KS);
+            const SeedRec* rp = srec + (cc.b * p.G4 + (int64_t)cc.tile * KS + pw) * 4;
 #pragma unroll
             for (int j = 0; j < kSeedGroups; ++j) {
-                if (pw + kSeedWarps * j < ngrp) {
+                if (pw + kSeedWarps * j < ng) {
                     const SeedRec* r = rp + kSeedWarps * j * 4;
-                    rt[j] = r->t; rcu[j] = r->cu; rsu[j] = r->su; rc4[j] = r->c4; rs4[j] = r->s4;
+                    nt_[j] = r->t; ncu[j] = r->cu; nsu[j] = r->su; ntc[j] = r->tcu;
                 }
             }
+        };
+        if (c.valid) fetch(c);
+        while (c.valid) {
+            const int ngrp = (int)min((int64_t)KS, p.G4 - (int64_t)c.tile * KS);
+            double rt[kSeedGroups], rcu[kSeedGroups], rsu[kSeedGroups], rtc[kSeedGroups];
+#pragma unroll
+            for (int j = 0; j < kSeedGroups; ++j) {
+                rt[j] = nt_[j]; rcu[j] = ncu[j]; rsu[j] = nsu[j]; rtc[j] = ntc[j];
+            }
+            const int nunits = c.n;
+            const int64_t u0 = c.u;
+            const double* tab_src = p.tab + ((c.b * p.n_pass + p.pass) * p.G4 + (int64_t)c.tile * KS) * GROUP;
+            c.advance(ntiles, U, CAP);
+            if (c.valid) fetch(c);
             if (!first_lap) mbar_wait(&bar_done[slot], par ^ 1u);
             unsigned char* base = smem_raw + slot * slot_bytes;
             if (pw == 0 && lane == 0) {
                 const uint32_t bytes = (uint32_t)ngrp * GROUP * 8u;
                 mbar_expect_tx(&bar_tab[slot], bytes);
-                bulk_g2s(base, p.tab + ((c.b * p.n_pass + p.pass) * p.G4 + (int64_t)c.tile * KS) * GROUP, bytes,
-                         &bar_tab[slot]);
+                bulk_g2s(base, tab_src, bytes, &bar_tab[slot]);
             }
             // centre of run m of the round's first unit: f_c = f0 + (run R + H - 1/2) df   (S1)
-            const double kc = (double)((c.u * 8 + m) * R + H) - 0.5;
+            const double kc = (double)((u0 * 8 + m) * R + H) - 0.5;
             const double fc = fma(kc, p.df, p.f0);
             double2* sb = reinterpret_cast<double2*>(base + tab_bytes) + lane;
 #pragma unroll
             for (int j = 0; j < kSeedGroups; ++j) {
                 const int ks = pw + kSeedWarps * j;
                 if (ks < ngrp) {
-                    double cs[CAP / 4], sn[CAP / 4];
-                    sincospi(2.0 * frac_prod(fc, rt[j]), &sn[0], &cs[0]);
-#pragma unroll
-                    for (int q = 1; q < CAP / 4; ++q) {  // units 4, 8, 12: rotations by four units
-                        cs[q] = cs[q - 1];
-                        sn[q] = sn[q - 1];
-                        rotate(cs[q], sn[q], rc4[j], rs4[j]);
-                    }
+                    // unit 0 exactly, unit 1 by one rotation, then the two-term recurrence
+                    // e_{u+1} = 2 cos(theta) e_u - e_{u-1} along the units (theta = one unit step)
+                    double c0, s0;
+                    sincos_turns(frac_prod(fc, rt[j]), trig64, c0, s0);
+                    double c1 = c0, s1 = s0;
+                    rotate(c1, s1, rcu[j], rsu[j]);
                     double2* dst = sb + (size_t)ks * CAP * 32;
+                    dst[0] = make_double2(c0, s0);
+                    dst[32] = make_double2(c1, s1);
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {  // units 4q + i: CAP/4 independent chains
-#pragma unroll
-                        for (int q = 0; q < CAP / 4; ++q) {
-                            dst[(4 * q + i) * 32] = make_double2(cs[q], sn[q]);
-                            if (i < 3) rotate(cs[q], sn[q], rcu[j], rsu[j]);
-                        }
+                    for (int u = 2; u < CAP; ++u) {
+                        if (u >= nunits) break;  // rounds of fewer units need fewer seeds
+                        const double c2 = fma(rtc[j], c1, -c0), s2 = fma(rtc[j], s1, -s0);
+                        dst[u * 32] = make_double2(c2, s2);
+                        c0 = c1;
+                        s0 = s1;
+                        c1 = c2;
+                        s1 = s2;
                     }
                 }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(&bar_seed[slot]);
-            c.advance(ntiles, U, CAP);
             if (++slot == NS) {
                 slot = 0;
                 par ^= 1u;
@@ -384,48 +502,56 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsMma));
         Tiles<H, NOCT, NB> acc;
         acc.clear();
-        int slot = 0;
-        uint32_t par = 0;
-        bool ready = false;  // the slot's barriers were seen complete one step ahead
-        while (c.valid) {
-            int off, cnt;
-            warp_share(c.n, wid, off, cnt);
-            if (!ready) {
-                mbar_wait(&bar_tab[slot], par);
-                mbar_wait(&bar_seed[slot], par);
+        RingPos rp = {0, 0u, false};
+        while (c.valid) {  // one round per iteration
+            const WarpRole role = warp_role(c.n, wid);
+#define FREDEC_ROUND(CNT) \
+    round_mma<CNT>(acc, rp, smem_raw, slot_bytes, tab_bytes, NS, KS, p.G4, role, lane, bar_tab, bar_seed, bar_done)
+            if (NOCT == 1 || role.cnt == 1) {
+                FREDEC_ROUND(1);
+            } else if (NOCT == 2 || role.cnt == 2) {
+                FREDEC_ROUND((NOCT >= 2 ? 2 : 1));
+            } else {
+                FREDEC_ROUND(NOCT);
             }
-            // look at the next slot's barriers now; the answer is needed after this step's MMAs
-            int nslot = slot + 1;
-            uint32_t npar = par;
-            if (nslot == NS) {
-                nslot = 0;
-                npar ^= 1u;
-            }
-            ready = mbar_test(&bar_tab[nslot], npar) & mbar_test(&bar_seed[nslot], npar);
-            if (cnt > 0) {
-                const unsigned char* base = smem_raw + slot * slot_bytes;
-                const double* tabs = reinterpret_cast<const double*>(base) + lane;
-                const double2* sb = reinterpret_cast<const double2*>(base + tab_bytes) + (size_t)off * 32 + lane;
-                const int ngrp = (int)min((int64_t)KS, p.G4 - (int64_t)c.tile * KS);
-                if (NOCT == 1 || cnt == 1) {
-                    mma_tile<1>(acc, tabs, sb, ngrp, CAP);
-                } else if (NOCT == 2 || cnt == 2) {
-                    mma_tile<(NOCT >= 2 ? 2 : 1)>(acc, tabs, sb, ngrp, CAP);
-                } else if (NOCT == 3 || cnt == 3) {
-                    mma_tile<(NOCT >= 3 ? 3 : 1)>(acc, tabs, sb, ngrp, CAP);
-                } else {
-                    mma_tile<NOCT>(acc, tabs, sb, ngrp, CAP);
+#undef FREDEC_ROUND
+            bool solve = true;
+            if (role.S > 1) {
+                // a8: the S warps of the unit add their partial sums in fixed order (sp = 1, 2, ...
+                // onto sp = 0) through the CTA's scratch in global memory; warp sp = 0 solves
+                constexpr int ACC1 = 2 * NF * NT * 2;
+                double* mine = p.red + ((size_t)blockIdx.x * kNW + wid) * (ACC1 * 32) + lane;
+                if (role.sp > 0) {
+#pragma unroll
+                    for (int x = 0; x < 2; ++x)
+#pragma unroll
+                        for (int f = 0; f < NF; ++f)
+#pragma unroll
+                            for (int t = 0; t < NT; ++t) {
+                                __stcg(mine + (((x * NF + f) * NT + t) * 2 + 0) * 32, acc.v[0][x][f][t][0]);
+                                __stcg(mine + (((x * NF + f) * NT + t) * 2 + 1) * 32, acc.v[0][x][f][t][1]);
+                            }
+                    solve = false;
+                }
+                asm volatile("bar.sync %0, %1;" ::"r"(1 + role.off), "r"(role.S * 32) : "memory");
+                if (role.sp == 0) {
+                    for (int sp = 1; sp < role.S; ++sp) {
+                        const double* other = mine + (size_t)sp * (ACC1 * 32);
+#pragma unroll
+                        for (int x = 0; x < 2; ++x)
+#pragma unroll
+                            for (int f = 0; f < NF; ++f)
+#pragma unroll
+                                for (int t = 0; t < NT; ++t) {
+                                    acc.v[0][x][f][t][0] += __ldcg(other + (((x * NF + f) * NT + t) * 2 + 0) * 32);
+                                    acc.v[0][x][f][t][1] += __ldcg(other + (((x * NF + f) * NT + t) * 2 + 1) * 32);
+                                }
+                    }
                 }
             }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&bar_done[slot]);
-            if (c.tile + 1 == ntiles && cnt > 0) {
-                solve_and_store<H, NOCT, NB>(acc, p, c.b, c.u + off, cnt, lane);
-                acc.clear();
-            }
-            c.advance(ntiles, U, CAP);
-            slot = nslot;
-            par = npar;
+            if (solve) solve_and_store<H, NOCT, NB>(acc, p, c.b, c.u + role.off, role.cnt, lane);
+            acc.clear();
+            c.next_round(U, CAP);
         }
     }
 }
@@ -465,6 +591,12 @@ size_t mma_scan_slot_bytes(int NB, int TI)
 {
     const MmaScanConfig c = mma_scan_config(NB);
     return (size_t)(TI / 4) * (mma_group_doubles(c.H, NB) * 8 + (size_t)(c.NW * c.NOCT) * 32 * 16);
+}
+
+size_t mma_red_doubles(int NB)
+{
+    const MmaScanConfig c = mma_scan_config(NB);
+    return (size_t)2 * mma_nf(NB) * mma_nt(c.H) * 2 * 32;
 }
 
 cudaError_t launch_mma_scan(int NB, const MmaScanParams& p, cudaStream_t stream)

@@ -23,9 +23,9 @@ __host__ __device__ constexpr int mma_nf(int NB) { return NB + 2; }
 __host__ __device__ constexpr int mma_group_doubles(int H, int NB) { return mma_nf(NB) * mma_nt(H) * 32; }
 
 // Per-observation seed record: t', (cos, sin) of the rotation by one unit (8 runs = 8R grid
-// steps) and by four units.
-struct __align__(16) SeedRec {
-    double t, cu, su, c4, s4, pad;
+// steps), and 2 cos of it (coefficient of the two-term recurrence along the units).
+struct __align__(32) SeedRec {
+    double t, cu, su, tcu;
 };
 
 struct MmaScanParams {
@@ -34,6 +34,7 @@ struct MmaScanParams {
     const SeriesInfo* info;  // [B]
     double* z;               // [B][K] out
     double* ws;              // [B][7][Kpad] partial sums between passes (nullptr if n_pass == 1)
+    double* red;             // [grid][MMA warps][mma_red_doubles] scratch of the observation-split reduction
     int64_t N, K, Kpad;
     int64_t G4;  // groups of 4 observations per series = ceil(N / 4)
     int64_t U;   // units per series = ceil(K / (8 R))
@@ -52,7 +53,8 @@ struct MmaScanConfig {
 // The (H, NOCT) the library is built with for NB base functions per pass (NB <= kMmaMaxNB).
 constexpr int kMmaMaxNB = 9;
 MmaScanConfig mma_scan_config(int NB);
-size_t mma_scan_slot_bytes(int NB, int TI);  // one ring slot; the kernel needs NS of them
+size_t mma_scan_slot_bytes(int NB, int TI);
+size_t mma_red_doubles(int NB);  // per MMA warp: the accumulators of one unit  // one ring slot; the kernel needs NS of them
 constexpr int kMmaMaxSlots = 8;
 cudaError_t launch_mma_scan(int NB, const MmaScanParams& p, cudaStream_t stream);
 
