@@ -158,6 +158,46 @@ def test_ragged_sizes(fr, oracle_mod, N, K):
     assert_parity(z, z_ref, f"N={N},K={K}")
 
 
+@pytest.mark.parametrize("d,units", [(2, 1), (2, 2), (2, 3), (2, 4), (2, 7), (2, 13), (1, 5), (0, 6), (3, 11), (9, 3), (9, 9)])
+def test_round_compositions_and_observation_split(fr, oracle_mod, d, units):
+    """Row a8: a grid of `units` 8-run MMA tiles is processed in rounds of 8, 4, 2 and 1 tiles; rounds of
+    fewer than 8 split the observations 2, 4 or 8 ways between warps and add the partial sums.  K is
+    chosen so that the last tile is ragged as well; N spans several ring slots and a ragged last one."""
+    run = 32 if d <= 2 else 16                 # frequencies per run (DESIGN.md section 5)
+    K = units * 8 * run - 5
+    t, x, w, base = inputs.random_series(9000 + 17 * d + units, 203, d)
+    f0, df = 0.003, 0.37 / K
+    z_ref = oracle_mod.scan(t, x, w, base, f0, df, K, threads=0)
+    z = gpu_scan(fr, t, x, w, base, f0, df, K)
+    assert_parity(z, z_ref, f"d={d},units={units}")
+
+
+def test_batched_short_series_split_rounds(fr, oracle_mod):
+    """Several series whose grids are shorter than one full round: every CTA runs split rounds,
+    and rounds never span two series."""
+    import torch
+    B, N, K = 37, 61, 700
+    ser = [inputs.random_series(4000 + b, N, 1) for b in range(B)]
+    t, x, w = (np.stack([s[i] for s in ser]) for i in range(3))
+    base = np.stack([s[3] for s in ser])
+    f0, df = 0.002, 0.0009
+    dt, dx, dw, db = _dev(t, x, w, base)
+    z = fr.fredec_scan_batched(dt, dx, dw, db, f0, df, K).cpu().numpy()
+    for b in range(B):
+        z_ref = oracle_mod.scan(t[b], x[b], w[b], base[b], f0, df, K, threads=0)
+        assert_parity(z[b], z_ref, f"series {b}")
+
+
+def test_bitwise_reproducible_runs(fr):
+    """Every accumulation order is fixed (S9): repeated runs of the survey-shaped workload, whose CTAs
+    end in split rounds, are bit-identical (a race in the shared-memory ring would show here)."""
+    wl = inputs.config(4, N=1500, K=150_000)
+    t, x, w, base = wl.series(0)
+    z0 = gpu_scan(fr, t, x, w, base, wl.f0, wl.df, wl.K)
+    for _ in range(4):
+        assert np.array_equal(z0, gpu_scan(fr, t, x, w, base, wl.f0, wl.df, wl.K))
+
+
 def test_host_and_device_pointers_agree_bitwise(fr):
     wl = inputs.config(2, K=5000)
     t, x, w, base = wl.series(0)
