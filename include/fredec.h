@@ -121,6 +121,65 @@ int fredec_scan_topk_batched(const double* t, const double* x, const double* w, 
                              const double* base_funcs, int32_t d, double f0, double df, int64_t K,
                              double* z_out, int32_t k, int64_t* idx_out);
 
+/* ------------------------------------------- statistic, FAP and the phase-1 driver */
+
+/*
+ * fredec_zstat -- the paper's statistic from the chi-square reduction (eq. 8,
+ * PAPER.md:106 eq. 10; reading G1: the printed ratio is read as the likelihood ratio
+ * l_base / l_alt):   z_out[k] = (N_H / 2) ln(chi2_base / (chi2_base - dchi2[k])).
+ *   dchi2 [K]   output of fredec_scan;  chi2_base > 0 from fredec_chi2_base;
+ *   N_H         N - dim H of the alternative: N - 3(m+1) - 1 when the base is a
+ *               constant + m sinusoids; in general N - d - (fitted base frequencies) - 3.  N_H > 0.
+ *   z_out [K]   may alias dchi2.  +inf where dchi2 == chi2_base (perfect fit).
+ */
+int fredec_zstat(const double* dchi2, int64_t K, double chi2_base, double N_H, double* z_out);
+
+/*
+ * fredec_fap1 -- single-frequency false alarm probability bound (eq. 13, n = 1):
+ *   fap_out[k] = min(1, A1 * W * exp(-z[k]) * sqrt(z[k]));  1 where z[k] <= 0.
+ *   W   = f_max * T_eff (fredec_bandwidth);  A1 = the coefficient A~_1, which this paper does not
+ *   print ("some numeric coefficients that we do not detail here"): the caller
+ *   supplies it (A1 > 0; 1.0 is the single-frequency bound of the Paper-I series).  fap_out may alias z.
+ */
+int fredec_fap1(const double* z, int64_t K, double W, double A1, double* fap_out);
+
+/*
+ * fredec_bandwidth -- T_eff = sqrt(4 pi Var(t_i)) with the weighted variance of the times, and
+ * W = f_max * T_eff.  t, w [N]; f_max >= 0; either output may be NULL.
+ */
+int fredec_bandwidth(const double* t, const double* w, int64_t N, double f_max, double* T_eff_out, double* W_out);
+
+/*
+ * fredec_phase1 -- phase 1 of FREDEC, the preliminary scan that builds the pool of candidate
+ * frequencies (section 4.2; SLICK + QUICK):
+ *   repeat: base model = constant + cos/sin pairs at the base frequencies found so far (all linear
+ *   coefficients refitted at every trial frequency, frequencies fixed: reading S4) -> residual
+ *   periodogram on the grid -> its k_peaks highest peaks -> statistic (fredec_zstat with
+ *   N_H = N - 3(m+1) - 1, m = base frequencies) and FAP (fredec_fap1, W from the grid's f_max).
+ *   Stop when the FAP of the highest peak exceeds fap0.  Otherwise every peak with FAP < fap1 AND
+ *   height >= half of the highest goes to the pool (a grid point already in the
+ *   pool keeps its smaller FAP), and the highest peak's frequency joins the base.
+ *   Finally the pool is cut to N/10 entries of smallest FAP.
+ * This build adds the GRID frequency of the peak to the base (no non-linear refinement, which is
+ * SURVEY 8(f) NEXT-3); DESIGN.md section 11 lists the readings.
+ *
+ *   t, x, w [N], f0, df, K        as fredec_scan (the base model is built internally)
+ *   fap0 <= fap1 in (0, 1]        thresholds (PAPER.md:228 defaults: 0.05 and 0.1);  A1 as fredec_fap1
+ *   max_base                      at most this many residual periodograms / base frequencies (>= 1,
+ *                                 2*max_base + 1 <= FREDEC_D_MAX)
+ *   k_peaks                       peaks examined per periodogram (1..FREDEC_TOPK_MAX)
+ *   pool_idx, pool_z, pool_fap [pool_cap]   HOST arrays: grid index, statistic and FAP of the pool,
+ *                                 sorted by FAP ascending then index; pool_cap >= 1
+ *   base_idx [max_base]           HOST array: grid indices of the base frequencies in the order found
+ *   n_base_out                    number of base frequencies
+ * Returns the pool size (<= min(pool_cap, N/10)), or a negative error code.
+ */
+int fredec_phase1(const double* t, const double* x, const double* w, int64_t N,
+                  double f0, double df, int64_t K,
+                  double fap0, double fap1, double A1, int32_t max_base, int32_t k_peaks,
+                  int64_t* pool_idx, double* pool_z, double* pool_fap, int32_t pool_cap,
+                  int64_t* base_idx, int32_t* n_base_out);
+
 /* ----------------------------------------------------------------- runtime control */
 
 /* Stream on which all work is enqueued (a cudaStream_t passed as void*); NULL = default. */

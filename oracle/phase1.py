@@ -1,0 +1,104 @@
+"""CPU oracle of the statistic, the single-frequency FAP and phase 1 of FREDEC (numpy + the C
+oracle's scan / topk).  TEST INFRASTRUCTURE ONLY (see oracle/__init__.py); shares no code with the
+CUDA path.  Each function follows the passage it cites, in the paper's order and notation.
+
+Pins (tests/test_oracle_pins.py): zstat against (N_H/2) ln(l_base/l_alt) with both l from QR fits;
+T_eff against the closed form for evenly spaced, equally weighted times; fap1 against hand values;
+phase 1 on constructed series whose outcome the rules fix.  The coefficient A~_1 of eq. 13 and the
+readings P1-P4 are not fixed by the paper: parity unpinned for those.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+from . import chi2_base as _chi2_base, scan as _scan, topk as _topk
+
+
+def zstat(dchi2, chi2_base: float, N_H: float):
+    """PAPER.md:89-95 (eq. 8) / :106 (eq. 10), reading G1: z = (N_H/2) ln(l_base / l_alt),
+    l_alt = l_base - dchi2."""
+    dchi2 = np.asarray(dchi2, dtype=np.float64)
+    l_alt = chi2_base - dchi2
+    with np.errstate(divide="ignore"):
+        return 0.5 * N_H * np.log(chi2_base / np.maximum(l_alt, 0.0))
+
+
+def fap1(z, W: float, A1: float = 1.0):
+    """PAPER.md:143 (eq. 13) with n = 1: FAP <~ A~_1 W e^{-z} z^{1/2}, capped at 1 (a probability)."""
+    z = np.asarray(z, dtype=np.float64)
+    zz = np.maximum(z, 0.0)
+    return np.where(z > 0.0, np.minimum(1.0, A1 * W * np.exp(-zz) * np.sqrt(zz)), 1.0)
+
+
+def bandwidth(t, w, f_max: float):
+    """T_eff = sqrt(4 pi Var(t_i)) with the weighted variance of t_i; W = f_max T_eff."""
+    t = np.asarray(t, dtype=np.float64)
+    w = np.asarray(w, dtype=np.float64)
+    mean = np.sum(w * t) / np.sum(w)
+    var = np.sum(w * (t - mean) ** 2) / np.sum(w)
+    T_eff = float(np.sqrt(4.0 * np.pi * var))
+    return T_eff, f_max * T_eff
+
+
+def sinusoid_base(t, freqs):
+    """PAPER.md:56 (eq. 2) with fixed frequencies: rows 1, cos 2 pi f_j t, sin 2 pi f_j t."""
+    t = np.asarray(t, dtype=np.float64)
+    rows = [np.ones_like(t)]
+    for f in freqs:
+        # the rounded product alone would lose the low bits of large phases: reduce exactly
+        hi = f * t
+        lo = np.array([_fma_residual(float(f), float(ti), float(h)) for ti, h in zip(t, hi)])
+        ph = 2.0 * np.pi * ((hi - np.rint(hi)) + lo)
+        rows.append(np.cos(ph))
+        rows.append(np.sin(ph))
+    return np.stack(rows)
+
+
+def _fma_residual(a: float, b: float, hi: float) -> float:
+    """a*b - hi exactly, in rational arithmetic (Python floats have no fma before 3.13)."""
+    from fractions import Fraction
+    return float(Fraction(a) * Fraction(b) - Fraction(hi))
+
+
+def _grid_frequency(f0: float, df: float, k: int) -> float:
+    """The double nearest f0 + k df (reading S1), as the C oracle's fma(k, df, f0)."""
+    from fractions import Fraction
+    return float(Fraction(k) * Fraction(df) + Fraction(f0))
+
+
+def phase1(t, x, w, f0, df, K, fap0=0.05, fap1_thr=0.1, A1=1.0, max_base=10, k_peaks=32, pool_cap=None,
+           threads: int = 0):
+    """PAPER.md:199-210 (section 4.2).  Returns dict(pool_idx, pool_z, pool_fap, base_idx)."""
+    t = np.asarray(t, dtype=np.float64)
+    N = t.shape[0]
+    pool_cap = max(1, N // 10) if pool_cap is None else pool_cap
+    f_max = f0 + df * (K - 1)
+    _, W = bandwidth(t, w, f_max)
+    base_f, base_idx, pool = [], [], {}
+    for m in range(max_base):
+        d = 2 * m + 1
+        N_H = N - 3 * (m + 1) - 1
+        if N_H <= 0 or N < d + 3:
+            break
+        base = sinusoid_base(t, base_f)
+        dchi2 = _scan(t, x, w, base, f0, df, K, threads=threads)  # "single-frequency residual periodogram"
+        l_base = _chi2_base(t, x, w, base)
+        idx, count = _topk(dchi2, k_peaks)
+        if count == 0 or not l_base > 0.0:
+            break
+        z = zstat(dchi2[idx[:count]], l_base, N_H)
+        fap = fap1(z, W, A1)
+        if fap[0] > fap0:
+            break
+        for j in range(count):
+            if j == 0 or (fap[j] < fap1_thr and z[j] >= 0.5 * z[0]):
+                i = int(idx[j])
+                if i not in pool or fap[j] < pool[i][1]:
+                    pool[i] = (float(z[j]), float(fap[j]))
+        base_idx.append(int(idx[0]))                            # "adding to the base model the frequency
+        base_f.append(_grid_frequency(f0, df, int(idx[0])))     #  corresponding to the largest peak"
+    entries = sorted(pool.items(), key=lambda kv: (kv[1][1], kv[0]))
+    entries = entries[:min(N // 10, pool_cap)]
+    return {"pool_idx": np.array([e[0] for e in entries], dtype=np.int64),
+            "pool_z": np.array([e[1][0] for e in entries]), "pool_fap": np.array([e[1][1] for e in entries]),
+            "base_idx": np.array(base_idx, dtype=np.int64)}

@@ -29,6 +29,11 @@ SIGNATURES = {
     "fredec_chi2_base_batched": (C.c_int, [_P, _P, _P, _I64, _I64, _P, _I32, _P]),
     "fredec_topk": (C.c_int, [_P, _I64, _I32, _P]),
     "fredec_topk_batched": (C.c_int, [_P, _I64, _I64, _I32, _P]),
+    "fredec_zstat": (C.c_int, [_P, _I64, _F64, _F64, _P]),
+    "fredec_fap1": (C.c_int, [_P, _I64, _F64, _F64, _P]),
+    "fredec_bandwidth": (C.c_int, [_P, _P, _I64, _F64, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    "fredec_phase1": (C.c_int, [_P, _P, _P, _I64, _F64, _F64, _I64, _F64, _F64, _F64, _I32, _I32,
+                                _P, _P, _P, _I32, _P, C.POINTER(C.c_int32)]),
     "fredec_set_stream": (C.c_int, [_P]),
     "fredec_last_timing": (C.c_int, [C.POINTER(C.c_double)]),
     "fredec_last_launches": (C.c_int, []),
@@ -200,6 +205,51 @@ def fredec_topk_batched(z, k, idx_out=None):
     pi, ki = _ptr(idx, np.int64)
     _check(lib().fredec_topk_batched(pz, B, K, int(k), pi), "fredec_topk_batched")
     return idx
+
+
+def fredec_zstat(dchi2, chi2_base, N_H, z_out=None):
+    """The paper's statistic z = (N_H/2) ln(chi2_base / (chi2_base - dchi2)); see include/fredec.h."""
+    K = int(dchi2.shape[-1])
+    z = _empty_like_kind(dchi2, (K,)) if z_out is None else z_out
+    (pi, ki), (po, ko) = _ptr(dchi2), _ptr(z)
+    _check(lib().fredec_zstat(pi, K, float(chi2_base), float(N_H), po), "fredec_zstat")
+    return z if z_out is None or ko is z else ko
+
+
+def fredec_fap1(z, W, A1=1.0, fap_out=None):
+    """Single-frequency FAP bound min(1, A1 W exp(-z) sqrt z); see include/fredec.h."""
+    K = int(z.shape[-1])
+    fap = _empty_like_kind(z, (K,)) if fap_out is None else fap_out
+    (pi, ki), (po, ko) = _ptr(z), _ptr(fap)
+    _check(lib().fredec_fap1(pi, K, float(W), float(A1), po), "fredec_fap1")
+    return fap if fap_out is None or ko is fap else ko
+
+
+def fredec_bandwidth(t, w, f_max):
+    """(T_eff, W) = (sqrt(4 pi Var_w t), f_max T_eff)."""
+    N = int(t.shape[-1])
+    te, W = C.c_double(), C.c_double()
+    (pt, kt), (pw, kw) = _ptr(t), _ptr(w)
+    _check(lib().fredec_bandwidth(pt, pw, N, float(f_max), C.byref(te), C.byref(W)), "fredec_bandwidth")
+    return te.value, W.value
+
+
+def fredec_phase1(t, x, w, f0, df, K, fap0=0.05, fap1=0.1, A1=1.0, max_base=10, k_peaks=32, pool_cap=None):
+    """Phase 1 of FREDEC (preliminary scan): returns a dict with the candidate pool (grid indices,
+    statistic, FAP; sorted by FAP) and the base frequencies' grid indices in the order found."""
+    N = int(t.shape[-1])
+    pool_cap = max(1, N // 10) if pool_cap is None else int(pool_cap)
+    pool_idx = np.empty(pool_cap, dtype=np.int64)
+    pool_z, pool_fap = np.empty(pool_cap), np.empty(pool_cap)
+    base_idx = np.empty(int(max_base), dtype=np.int64)
+    n_base = C.c_int32(0)
+    (pt, kt), (px, kx), (pw, kw) = map(_ptr, (t, x, w))
+    n = _check(lib().fredec_phase1(pt, px, pw, N, float(f0), float(df), int(K), float(fap0), float(fap1),
+                                   float(A1), int(max_base), int(k_peaks), pool_idx.ctypes.data,
+                                   pool_z.ctypes.data, pool_fap.ctypes.data, pool_cap, base_idx.ctypes.data,
+                                   C.byref(n_base)), "fredec_phase1")
+    return {"pool_idx": pool_idx[:n].copy(), "pool_z": pool_z[:n].copy(), "pool_fap": pool_fap[:n].copy(),
+            "base_idx": base_idx[:n_base.value].copy()}
 
 
 def fredec_last_timing() -> dict:

@@ -5,12 +5,15 @@
 #include <cstdint>
 #include <cstdlib>
 #include <cstring>
+#include <algorithm>
+#include <vector>
 #include <cuda_runtime.h>
 
 #include "fredec.h"
 #include "peak_kernel.cuh"
 #include "prep_kernel.cuh"
 #include "scan_mma_kernel.cuh"
+#include "stat_kernel.cuh"
 #include "topk_kernel.cuh"
 
 using namespace fredec;
@@ -74,7 +77,7 @@ struct State {
     cudaStream_t stream = nullptr;
     cudaEvent_t ev[kNumEvents] = {};
     DevBuf in_t, in_x, in_w, in_base, in_z, out_z, out_idx, out_chi2;
-    DevBuf tab, srec, psi, xt, info, ws, red, part_z, part_i, count, sink;
+    DevBuf p1_base, p1_freq, p1_z, p1_idx, p1_stats, tab, srec, psi, xt, info, ws, red, part_z, part_i, count, sink;
     HostBuf h_info, h_count;
     int last_cuda = 0;
     double timing[4] = {0, 0, 0, 0};
@@ -443,6 +446,41 @@ int do_topk(const double* z, int64_t B, int64_t K, int32_t k, int64_t* idx_out, 
     return finish_call(c, first_count);
 }
 
+// element-wise map of a [K] array (zstat / fap1): stage, launch, copy out, one sync
+template <class Launch>
+int do_map(const double* in, int64_t K, double* out, Launch launch)
+{
+    if (!in || !out || K < 1) return FREDEC_EINVAL;
+    int rc = begin_call();
+    if (rc) return rc;
+    const double* din;
+    if ((rc = stage_in(in, (size_t)K, g.in_z, &din))) return rc;
+    double *dout, *hout;
+    if ((rc = stage_out(out, (size_t)K, g.out_z, &dout, &hout))) return rc;
+    CK(launch(din, dout, g.stream));
+    g.launches += 1;
+    if (hout) CK(cudaMemcpyAsync(hout, dout, (size_t)K * 8, cudaMemcpyDeviceToHost, g.stream));
+    CK(cudaEventRecord(g.ev[6], g.stream));
+    CK(cudaStreamSynchronize(g.stream));
+    g.timing[3] = ev_ms(0, 6);
+    return FREDEC_OK;
+}
+
+// T_eff, weighted variance and mean of t; dt, dw device pointers
+int device_bandwidth(const double* dt, const double* dw, int64_t N, double out4[4])
+{
+    CK(g.sink.reserve(64));
+    CK(launch_bandwidth(dt, dw, N, g.sink.as<double>(), g.stream));
+    CK(cudaMemcpyAsync(out4, g.sink.p, 32, cudaMemcpyDeviceToHost, g.stream));
+    CK(cudaStreamSynchronize(g.stream));
+    return out4[3] != 0.0 ? FREDEC_EDATA : FREDEC_OK;
+}
+
+struct PoolEntry {
+    int64_t idx;
+    double z, fap;
+};
+
 }  // namespace
 
 extern "C" {
@@ -496,6 +534,125 @@ int fredec_topk_batched(const double* z, int64_t B, int64_t K, int32_t k, int64_
     return do_topk(z, B, K, k, idx_out, nullptr);
 }
 
+int fredec_zstat(const double* dchi2, int64_t K, double chi2_base, double N_H, double* z_out)
+{
+    if (!(chi2_base > 0.0) || !std::isfinite(chi2_base) || !(N_H > 0.0) || !std::isfinite(N_H)) return FREDEC_EINVAL;
+    return do_map(dchi2, K, z_out, [&](const double* in, double* out, cudaStream_t st) {
+        return launch_zstat(in, K, chi2_base, N_H, out, st);
+    });
+}
+
+int fredec_fap1(const double* z, int64_t K, double W, double A1, double* fap_out)
+{
+    if (!(W >= 0.0) || !std::isfinite(W) || !(A1 > 0.0) || !std::isfinite(A1)) return FREDEC_EINVAL;
+    return do_map(z, K, fap_out, [&](const double* in, double* out, cudaStream_t st) {
+        return launch_fap1(in, K, W, A1, out, st);
+    });
+}
+
+int fredec_bandwidth(const double* t, const double* w, int64_t N, double f_max, double* T_eff_out, double* W_out)
+{
+    if (!t || !w || N < 2 || !(f_max >= 0.0) || !std::isfinite(f_max)) return FREDEC_EINVAL;
+    int rc = begin_call();
+    if (rc) return rc;
+    const double *dt, *dw;
+    if ((rc = stage_in(t, (size_t)N, g.in_t, &dt))) return rc;
+    if ((rc = stage_in(w, (size_t)N, g.in_w, &dw))) return rc;
+    double out4[4];
+    if ((rc = device_bandwidth(dt, dw, N, out4))) return rc;
+    g.launches += 1;
+    if (T_eff_out) *T_eff_out = out4[0];
+    if (W_out) *W_out = f_max * out4[0];
+    return FREDEC_OK;
+}
+
+int fredec_phase1(const double* t, const double* x, const double* w, int64_t N, double f0, double df, int64_t K,
+                  double fap0, double fap1, double A1, int32_t max_base, int32_t k_peaks, int64_t* pool_idx,
+                  double* pool_z, double* pool_fap, int32_t pool_cap, int64_t* base_idx, int32_t* n_base_out)
+{
+    if (!t || !x || !w || !pool_idx || !pool_z || !pool_fap || !base_idx || !n_base_out) return FREDEC_EINVAL;
+    if (N < 4 || pool_cap < 1 || max_base < 1 || 2 * max_base + 1 > FREDEC_D_MAX) return FREDEC_EINVAL;
+    if (!(fap0 > 0.0) || !(fap1 <= 1.0) || !(fap0 <= fap1) || !(A1 > 0.0) || !std::isfinite(A1)) return FREDEC_EINVAL;
+    int rc = check_grid_args(f0, df, K);
+    if (rc) return rc;
+    if ((rc = check_topk_args(1, K, k_peaks))) return rc;
+    if (on_device(pool_idx) || on_device(pool_z) || on_device(pool_fap) || on_device(base_idx)) return FREDEC_EINVAL;
+    if ((rc = ensure_ready())) return rc;
+    cudaStream_t st = g.stream;
+
+    // the series stays on the device for all iterations
+    const double *dt, *dx, *dw;
+    if ((rc = stage_in(t, (size_t)N, g.in_t, &dt))) return rc;
+    if ((rc = stage_in(x, (size_t)N, g.in_x, &dx))) return rc;
+    if ((rc = stage_in(w, (size_t)N, g.in_w, &dw))) return rc;
+    double bw[4];
+    if ((rc = device_bandwidth(dt, dw, N, bw))) return rc;
+    const double f_max = f0 + df * (double)(K - 1);
+    const double W = f_max * bw[0];  // W = f_max T_eff
+
+    CK(g.p1_base.reserve((size_t)(2 * max_base + 1) * N * 8));
+    CK(g.p1_freq.reserve((size_t)max_base * 8));
+    CK(g.p1_z.reserve((size_t)K * 8));
+    CK(g.p1_idx.reserve((size_t)k_peaks * 8));
+    CK(g.p1_stats.reserve((size_t)k_peaks * 16));
+    std::vector<double> base_f, stats(2 * (size_t)k_peaks);
+    std::vector<int64_t> idx((size_t)k_peaks);
+    std::vector<PoolEntry> pool;
+    int launches = 1;
+    *n_base_out = 0;
+
+    for (int m = 0; m < max_base; ++m) {
+        const int d = 2 * m + 1;
+        const double NH = (double)N - 3.0 * (m + 1) - 1.0;  // N - dim H_{m+1}
+        if (NH <= 0.0 || N < (int64_t)d + 3) break;
+        if (m > 0) CK(cudaMemcpyAsync(g.p1_freq.p, base_f.data(), (size_t)m * 8, cudaMemcpyHostToDevice, st));
+        CK(launch_sin_base(dt, N, g.p1_freq.as<double>(), m, g.p1_base.as<double>(), st));
+        const int count = do_scan(dt, dx, dw, 1, N, g.p1_base.as<double>(), d, f0, df, K, g.p1_z.as<double>(), k_peaks,
+                                  g.p1_idx.as<int64_t>(), true);
+        launches += 1 + g.launches;
+        if (count < 0) return count;
+        if (count == 0) break;
+        const double chi2_base = static_cast<const SeriesInfo*>(g.h_info.p)[0].chi2_base;
+        if (!(chi2_base > 0.0)) break;  // the base model already fits exactly
+        CK(launch_peak_stats(g.p1_z.as<double>(), g.p1_idx.as<int64_t>(), k_peaks, chi2_base, NH, W, A1,
+                             g.p1_stats.as<double>(), st));
+        launches += 1;
+        CK(cudaMemcpyAsync(idx.data(), g.p1_idx.p, (size_t)k_peaks * 8, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(stats.data(), g.p1_stats.p, (size_t)k_peaks * 16, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        const double z_top = stats[0], fap_top = stats[1];
+        if (fap_top > fap0) break;
+        for (int j = 0; j < count; ++j) {
+            const double zj = stats[2 * j], fj = stats[2 * j + 1];
+            const bool take = j == 0 || (fj < fap1 && zj >= 0.5 * z_top);
+            if (!take) continue;
+            auto it = std::find_if(pool.begin(), pool.end(), [&](const PoolEntry& e) { return e.idx == idx[j]; });
+            if (it == pool.end()) {
+                pool.push_back(PoolEntry{idx[j], zj, fj});
+            } else if (fj < it->fap) {
+                it->z = zj;
+                it->fap = fj;
+            }
+        }
+        base_idx[m] = idx[0];
+        base_f.push_back(std::fma((double)idx[0], df, f0));
+        *n_base_out = m + 1;
+    }
+    std::sort(pool.begin(), pool.end(), [](const PoolEntry& a, const PoolEntry& b) {
+        return a.fap < b.fap || (a.fap == b.fap && a.idx < b.idx);
+    });
+    size_t n = pool.size();
+    if (n > (size_t)(N / 10)) n = (size_t)(N / 10);
+    if (n > (size_t)pool_cap) n = (size_t)pool_cap;
+    for (size_t i = 0; i < n; ++i) {
+        pool_idx[i] = pool[i].idx;
+        pool_z[i] = pool[i].z;
+        pool_fap[i] = pool[i].fap;
+    }
+    g.launches = launches;
+    return (int)n;
+}
+
 int fredec_set_stream(void* cuda_stream)
 {
     g.stream = static_cast<cudaStream_t>(cuda_stream);
@@ -532,7 +689,7 @@ int fredec_fp64_peak(int64_t iters, double* tflops_out, double* ms_out)
 
 int fredec_shutdown(void)
 {
-    DevBuf* bufs[] = {&g.in_t, &g.in_x, &g.in_w, &g.in_base, &g.in_z, &g.out_z, &g.out_idx, &g.out_chi2, &g.tab, &g.srec,
+    DevBuf* bufs[] = {&g.in_t, &g.in_x, &g.in_w, &g.in_base, &g.in_z, &g.out_z, &g.out_idx, &g.out_chi2, &g.p1_base, &g.p1_freq, &g.p1_z, &g.p1_idx, &g.p1_stats, &g.tab, &g.srec,
                       &g.psi,  &g.xt,   &g.info, &g.ws, &g.red,     &g.part_z, &g.part_i, &g.count, &g.sink};
     for (DevBuf* b : bufs) b->release();
     g.h_info.release();

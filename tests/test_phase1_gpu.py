@@ -1,0 +1,109 @@
+"""GPU parity of the statistic, FAP, bandwidth and phase-1 entry points
+against oracle/phase1.py, through the C-ABI binding.  Integer results (grid indices, counts)
+must be identical; floating point within 1e-12 relative (element-wise maps: a handful of
+correctly rounded operations) and 1e-9 relative for statistics derived from a scan."""
+import numpy as np
+import pytest
+
+from paper_1309_0100_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def fr():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1309_0100_b200 import build
+    build.build()
+    import paper_1309_0100_b200 as fr
+    fr.lib()
+    return fr
+
+
+@pytest.fixture(scope="module")
+def p1(oracle_mod):
+    from oracle import phase1
+    return phase1
+
+
+@pytest.mark.parametrize("K", [1, 7, 1000, 300_001])
+def test_zstat_and_fap1_elementwise(fr, p1, K):
+    import torch
+    rng = np.random.Generator(np.random.PCG64(K))
+    chi2 = 123.456
+    dchi2 = chi2 * rng.uniform(0.0, 0.999, K)
+    dchi2[0] = 0.0
+    z_ref = p1.zstat(dchi2, chi2, 57.0)
+    z = fr.fredec_zstat(dchi2, chi2, 57.0)                               # host pointers
+    assert np.max(np.abs(z - z_ref)) <= 1e-12 * np.max(z_ref) + 1e-300
+    zd = fr.fredec_zstat(torch.from_numpy(dchi2).cuda(), chi2, 57.0)     # device pointers
+    assert np.array_equal(zd.cpu().numpy(), z)
+    fap_ref = p1.fap1(z, 35.5, 0.8)                                     # the same z on both sides
+    fap = fr.fredec_fap1(z, 35.5, 0.8)
+    assert np.all(np.abs(fap - fap_ref) <= 1e-13 * fap_ref + 1e-300)       # exp, sqrt: a few ulp
+    assert fap[0] == 1.0 and np.all(fap <= 1.0) and np.all(fap >= 0.0)
+
+
+def test_zstat_perfect_fit_is_inf(fr):
+    z = fr.fredec_zstat(np.array([5.0, 2.5]), 5.0, 10.0)
+    assert np.isinf(z[0]) and z[0] > 0 and abs(z[1] - 5.0 * np.log(2.0)) < 1e-14
+
+
+def test_bandwidth_parity(fr, p1):
+    for cfg in (1, 2, 4):
+        wl = inputs.config(cfg)
+        t, x, w, _ = wl.series(0)
+        f_max = wl.f0 + wl.df * (wl.K - 1)
+        T_ref, W_ref = p1.bandwidth(t, w, f_max)
+        T, W = fr.fredec_bandwidth(t, w, f_max)
+        assert abs(T - T_ref) <= 1e-12 * T_ref and abs(W - W_ref) <= 1e-12 * W_ref
+
+
+def _assert_phase1_equal(r, ref):
+    assert r["base_idx"].tolist() == ref["base_idx"].tolist()
+    assert r["pool_idx"].tolist() == ref["pool_idx"].tolist()
+    assert np.all(np.abs(r["pool_z"] - ref["pool_z"]) <= 1e-9 * np.abs(ref["pool_z"]))
+    assert np.all(np.abs(r["pool_fap"] - ref["pool_fap"]) <= 1e-7 * ref["pool_fap"] + 1e-300)
+
+
+def test_phase1_rv_like_series(fr, p1):
+    """Config-2 shaped series (seasonal gaps, five sinusoids): several SLICK iterations with alias
+    side peaks; pool and base frequencies identical to the oracle's."""
+    wl = inputs.config(2, N=400, K=40_000)
+    t, x, w, _ = wl.series(0)
+    kw = dict(fap0=0.05, fap1=0.1, A1=1.0, max_base=8, k_peaks=24)
+    ref = p1.phase1(t, x, w, wl.f0, wl.df, wl.K, fap0=0.05, fap1_thr=0.1, A1=1.0, max_base=8, k_peaks=24)
+    r = fr.fredec_phase1(t, x, w, wl.f0, wl.df, wl.K, **kw)
+    assert len(ref["base_idx"]) >= 2
+    _assert_phase1_equal(r, ref)
+    import torch
+    rd = fr.fredec_phase1(*[torch.from_numpy(a).cuda() for a in (t, x, w)], wl.f0, wl.df, wl.K, **kw)
+    _assert_phase1_equal(rd, r)
+
+
+def test_phase1_tiny_config_and_noise(fr, p1):
+    wl = inputs.config(1)
+    t, x, w, _ = wl.series(0)
+    ref = p1.phase1(t, x, w, wl.f0, wl.df, wl.K, max_base=5, k_peaks=10)
+    r = fr.fredec_phase1(t, x, w, wl.f0, wl.df, wl.K, max_base=5, k_peaks=10)
+    _assert_phase1_equal(r, ref)
+    assert abs(1.0 / (wl.f0 + r["base_idx"][0] * wl.df) - 17.3) < 0.1      # the generator's main period
+    rng = np.random.Generator(np.random.PCG64(12))
+    tn = np.sort(rng.uniform(0.0, 100.0, 80))
+    xn = rng.standard_normal(80)
+    rn = fr.fredec_phase1(tn, xn, np.ones(80), 0.005, 0.001, 2000, fap0=0.01, fap1=0.02)
+    assert rn["base_idx"].size == 0 and rn["pool_idx"].size == 0
+
+
+def test_phase1_argument_errors(fr):
+    t, x, w, _ = inputs.random_series(1, 50, 0)
+    with pytest.raises(fr.FredecError) as e:
+        fr.fredec_phase1(t, x, w, 0.01, 0.001, 100, fap0=0.2, fap1=0.1)      # FAP_1 >= FAP_0
+    assert e.value.code == fr.FREDEC_EINVAL
+    with pytest.raises(fr.FredecError):
+        fr.fredec_phase1(t, x, w, 0.01, 0.001, 100, max_base=40)            # 2*40+1 > FREDEC_D_MAX
+    with pytest.raises(fr.FredecError):
+        fr.fredec_zstat(np.ones(4), -1.0, 10.0)
+    with pytest.raises(fr.FredecError):
+        fr.fredec_fap1(np.ones(4), 1.0, 0.0)
