@@ -180,6 +180,19 @@ int fredec_phase1(const double* t, const double* x, const double* w, int64_t N,
                   int64_t* pool_idx, double* pool_z, double* pool_fap, int32_t pool_cap,
                   int64_t* base_idx, int32_t* n_base_out);
 
+/*
+ * fredec_trig_averages -- the trigonometric averages behind the gradient and Fisher matrix of the
+ * local multifrequency fit (section 5, systems (19) and (20)) at an ARBITRARY list
+ * of M frequencies f_j (omega_j = 2 pi f_j; for system (20) the caller passes the sums and
+ * differences f_k +- f_m).  out [M][10], row j, in the paper's order:
+ *   system (19):  <cos wt> <sin wt> <t cos wt> <t sin wt> <x cos wt> <x sin wt> <x t cos wt> <x t sin wt>
+ *   system (20):  columns 0..3 again, then  <t^2 cos wt> <t^2 sin wt>   (columns 8, 9)
+ * with <phi> = sum_i w_i phi(t_i) and t used as given (the paper centres it so that
+ * <t> = 0).  t, x, w [N]; freqs [M], finite; M <= 2^31 - 1.
+ */
+int fredec_trig_averages(const double* t, const double* x, const double* w, int64_t N,
+                         const double* freqs, int64_t M, double* out);
+
 /* ----------------------------------------------------------------- runtime control */
 
 /* Stream on which all work is enqueued (a cudaStream_t passed as void*); NULL = default. */

@@ -25,6 +25,9 @@ def lib():
             f = getattr(L, "oracle_chi2_base" + sfx)
             f.restype = C.c_int
             f.argtypes = [_f64p, _f64p, _f64p, C.c_int64, C.c_void_p, C.c_int32, _f64p]
+            f = getattr(L, "oracle_trig_averages" + sfx)
+            f.restype = C.c_int
+            f.argtypes = [_f64p, _f64p, _f64p, C.c_int64, _f64p, C.c_int64, _f64p]
         L.oracle_topk.restype = C.c_int
         L.oracle_topk.argtypes = [_f64p, C.c_int64, C.c_int32, _i64p]
         L.oracle_num_threads.restype = C.c_int
@@ -74,6 +77,20 @@ def chi2_base(t, x, w, base_funcs, long_double: bool = False):
     if rc != 0:
         raise RuntimeError(f"oracle_chi2_base failed with code {rc}")
     return float(out[0])
+
+
+def trig_averages(t, x, w, freqs, long_double: bool = False):
+    """[M][10] trigonometric averages of PAPER.md:242-262, systems (19) and (20), at the given
+    frequencies (cycles per unit of t); column order in oracle_fredec.c."""
+    L = lib()
+    t, x, w = (np.ascontiguousarray(a, dtype=np.float64) for a in (t, x, w))
+    freqs = np.ascontiguousarray(freqs, dtype=np.float64)
+    out = np.empty((freqs.shape[0], 10), dtype=np.float64)
+    fn = L.oracle_trig_averages_ld if long_double else L.oracle_trig_averages
+    rc = fn(t, x, w, t.shape[0], freqs, freqs.shape[0], out)
+    if rc != 0:
+        raise RuntimeError(f"oracle_trig_averages failed with code {rc}")
+    return out
 
 
 def topk(z, k):

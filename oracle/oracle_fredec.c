@@ -246,6 +246,35 @@ int FN(oracle_scan_batched)(const double *t, const double *x, const double *w, i
     return ORACLE_OK;
 }
 
+/* Trigonometric averages of PAPER.md:242-262 (section 5) at an arbitrary list of M frequencies
+ * (omega_j = 2 pi f_j), per pair with libm on the exactly reduced phase, summed in index order.
+ * out [M][10], in the paper's order: system (19)
+ *   0 <cos wt>   1 <sin wt>   2 <t cos wt>   3 <t sin wt>
+ *   4 <x cos wt> 5 <x sin wt> 6 <x t cos wt> 7 <x t sin wt>
+ * and the two further averages of system (20) (its first four are 0..3 above)
+ *   8 <t^2 cos wt>  9 <t^2 sin wt>.
+ * <phi> = sum_i w_i phi(t_i); t is used as given (the paper sets <t> = 0). */
+int FN(oracle_trig_averages)(const double *t, const double *x, const double *w, int64_t N,
+                             const double *freqs, int64_t M, double *out)
+{
+    if (!t || !x || !w || !freqs || !out || N < 1 || M < 1) return ORACLE_EINVAL;
+    for (int64_t j = 0; j < M; ++j) {
+        real a[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+        for (int64_t i = 0; i < N; ++i) {
+            real c, s;
+            trial_pair((real)freqs[j], (real)t[i], &c, &s);
+            const real wi = w[i], ti = t[i], xi = x[i];
+            a[0] += wi * c;            a[1] += wi * s;
+            a[2] += wi * ti * c;       a[3] += wi * ti * s;
+            a[4] += wi * xi * c;       a[5] += wi * xi * s;
+            a[6] += wi * xi * ti * c;  a[7] += wi * xi * ti * s;
+            a[8] += wi * ti * ti * c;  a[9] += wi * ti * ti * s;
+        }
+        for (int q = 0; q < 10; ++q) out[j * 10 + q] = (double)a[q];
+    }
+    return ORACLE_OK;
+}
+
 #ifdef ORACLE_IS_DOUBLE
 /* Peaks (S7): k is a peak iff z[k] > z[k-1] and z[k] >= z[k+1], neighbours outside the
  * grid count as -infinity, NaN counts as -infinity.  Ranked by z descending, then index

@@ -34,6 +34,7 @@ SIGNATURES = {
     "fredec_bandwidth": (C.c_int, [_P, _P, _I64, _F64, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "fredec_phase1": (C.c_int, [_P, _P, _P, _I64, _F64, _F64, _I64, _F64, _F64, _F64, _I32, _I32,
                                 _P, _P, _P, _I32, _P, C.POINTER(C.c_int32)]),
+    "fredec_trig_averages": (C.c_int, [_P, _P, _P, _I64, _P, _I64, _P]),
     "fredec_set_stream": (C.c_int, [_P]),
     "fredec_last_timing": (C.c_int, [C.POINTER(C.c_double)]),
     "fredec_last_launches": (C.c_int, []),
@@ -250,6 +251,15 @@ def fredec_phase1(t, x, w, f0, df, K, fap0=0.05, fap1=0.1, A1=1.0, max_base=10, 
                                    C.byref(n_base)), "fredec_phase1")
     return {"pool_idx": pool_idx[:n].copy(), "pool_z": pool_z[:n].copy(), "pool_fap": pool_fap[:n].copy(),
             "base_idx": base_idx[:n_base.value].copy()}
+
+
+def fredec_trig_averages(t, x, w, freqs, out=None):
+    """[M][10] trigonometric averages of the paper's systems (19) and (20); see include/fredec.h."""
+    N, M = int(t.shape[-1]), int(freqs.shape[-1])
+    res = _empty_like_kind(t, (M, 10)) if out is None else out
+    (pt, kt), (px, kx), (pw, kw), (pf, kf), (po, ko) = map(_ptr, (t, x, w, freqs, res))
+    _check(lib().fredec_trig_averages(pt, px, pw, N, pf, M, po), "fredec_trig_averages")
+    return res if out is None or ko is res else ko
 
 
 def fredec_last_timing() -> dict:

@@ -14,6 +14,7 @@
 #include "prep_kernel.cuh"
 #include "scan_mma_kernel.cuh"
 #include "stat_kernel.cuh"
+#include "trig_kernel.cuh"
 #include "topk_kernel.cuh"
 
 using namespace fredec;
@@ -651,6 +652,28 @@ int fredec_phase1(const double* t, const double* x, const double* w, int64_t N, 
     }
     g.launches = launches;
     return (int)n;
+}
+
+int fredec_trig_averages(const double* t, const double* x, const double* w, int64_t N, const double* freqs, int64_t M,
+                         double* out)
+{
+    if (!t || !x || !w || !freqs || !out || N < 1 || M < 1 || M > 0x7fffffff) return FREDEC_EINVAL;
+    int rc = begin_call();
+    if (rc) return rc;
+    const double *dt, *dx, *dw, *dfr;
+    if ((rc = stage_in(t, (size_t)N, g.in_t, &dt))) return rc;
+    if ((rc = stage_in(x, (size_t)N, g.in_x, &dx))) return rc;
+    if ((rc = stage_in(w, (size_t)N, g.in_w, &dw))) return rc;
+    if ((rc = stage_in(freqs, (size_t)M, g.in_z, &dfr))) return rc;
+    double *dout, *hout;
+    if ((rc = stage_out(out, (size_t)M * kTrigCols, g.out_z, &dout, &hout))) return rc;
+    CK(launch_trig_averages(dt, dx, dw, N, dfr, M, dout, g.stream));
+    g.launches += 1;
+    if (hout) CK(cudaMemcpyAsync(hout, dout, (size_t)M * kTrigCols * 8, cudaMemcpyDeviceToHost, g.stream));
+    CK(cudaEventRecord(g.ev[6], g.stream));
+    CK(cudaStreamSynchronize(g.stream));
+    g.timing[3] = ev_ms(0, 6);
+    return FREDEC_OK;
 }
 
 int fredec_set_stream(void* cuda_stream)

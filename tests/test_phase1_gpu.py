@@ -107,3 +107,23 @@ def test_phase1_argument_errors(fr):
         fr.fredec_zstat(np.ones(4), -1.0, 10.0)
     with pytest.raises(fr.FredecError):
         fr.fredec_fap1(np.ones(4), 1.0, 0.0)
+
+
+@pytest.mark.parametrize("N,M", [(1, 1), (37, 5), (1000, 300), (10_000, 25)])
+def test_trig_averages_parity(fr, oracle_mod, N, M):
+    """Systems (19), (20) of PAPER.md:242-262 at an arbitrary frequency list.  Tolerance: every term
+    carries a few ulp (sincos, products) and the N-term sums differ in order: 4 N eps x sum |term|."""
+    import torch
+    rng = np.random.Generator(np.random.PCG64(1000 * N + M))
+    t = np.sort(rng.uniform(-1500.0, 1500.0, N))
+    x = rng.standard_normal(N) * 3.0 + 1.0
+    w = rng.uniform(0.25, 4.0, N)
+    freqs = rng.uniform(0.0, 3.0, M)
+    freqs[0] = 0.0
+    ref = oracle_mod.trig_averages(t, x, w, freqs)
+    got = fr.fredec_trig_averages(t, x, w, freqs)
+    s1, st, sx, sxt, st2 = (np.sum(w * a) for a in (1.0 + 0 * t, abs(t), abs(x), abs(x * t), t * t))
+    scale = np.array([s1, s1, st, st, sx, sx, sxt, sxt, st2, st2])
+    assert np.all(np.abs(got - ref) <= 4 * N * np.finfo(float).eps * scale + 1e-300)
+    gd = fr.fredec_trig_averages(*[torch.from_numpy(a).cuda() for a in (t, x, w, freqs)])
+    assert np.array_equal(gd.cpu().numpy(), got)
