@@ -10,13 +10,20 @@
 // one comparison; the rare survivors are inserted with warp shuffles.  Warp lists are merged
 // per CTA through shared memory, CTA lists by a second small kernel.  No atomics.
 #include <cmath>
+#include <cstdint>
 #include "topk_kernel.cuh"
 
 namespace fredec {
 
 namespace {
 
-constexpr int kTopkThreads = 256;
+#ifndef FREDEC_TOPK_THREADS
+#define FREDEC_TOPK_THREADS 256
+#endif
+#ifndef FREDEC_TOPK_UN
+#define FREDEC_TOPK_UN 4
+#endif
+constexpr int kTopkThreads = FREDEC_TOPK_THREADS;
 constexpr int kTopkWarps = kTopkThreads / 32;
 constexpr int64_t kEmptyIdx = INT64_MAX;
 
@@ -154,25 +161,59 @@ __global__ void __launch_bounds__(kTopkThreads) topk_scan_kernel(TopkParams p)
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t b = blockIdx.y, K = p.K;
     const double* z = p.z + b * K;
-    // contiguous chunk of this CTA, a multiple of the CTA width
+    // contiguous chunk of this CTA, a multiple of what the CTA covers per step
+    constexpr int UN = FREDEC_TOPK_UN;                               // 16-byte loads in flight per thread
+    constexpr int64_t kStep = kTopkThreads * 2;         // elements per CTA and sub-step
     int64_t chunk = (K + p.nblk - 1) / p.nblk;
-    chunk = (chunk + kTopkThreads - 1) / kTopkThreads * kTopkThreads;
+    chunk = (chunk + kStep - 1) / kStep * kStep;
     const int64_t begin = (int64_t)blockIdx.x * chunk;
     const int64_t end = min(K, begin + chunk);
 
     WarpList<SLOTS> L;
     L.init(p.k, lane);
-    for (int64_t base = begin + wid * 32; base < end; base += kTopkThreads) {
-        const int64_t i = base + lane;
-        bool peak = false;
-        double v = -INFINITY;
-        if (i < K) {
-            v = sanitize(z[i]);
-            const double l = i > 0 ? sanitize(z[i - 1]) : -INFINITY;
-            const double r = i + 1 < K ? sanitize(z[i + 1]) : -INFINITY;
-            peak = v > l && v >= r;
+    if ((reinterpret_cast<uintptr_t>(z) & 15) == 0) {
+        // each lane owns two adjacent elements per sub-step (one 16-byte load); their outer
+        // neighbours come from the adjacent lanes, the warp's two outer neighbours from L1/L2
+        for (int64_t base = begin + wid * 64; base < end; base += kStep * UN) {
+            double2 v[UN];
+            double lft[UN], rgt[UN];
+#pragma unroll
+            for (int u = 0; u < UN; ++u) {
+                const int64_t i0 = base + u * kStep + 2 * lane;
+                v[u] = make_double2(-INFINITY, -INFINITY);
+                if (i0 + 1 < K) {
+                    v[u] = *reinterpret_cast<const double2*>(z + i0);
+                } else if (i0 < K) {
+                    v[u].x = z[i0];
+                }
+                lft[u] = (lane == 0 && i0 > 0 && i0 < K) ? z[i0 - 1] : -INFINITY;
+                rgt[u] = (lane == 31 && i0 + 2 < K) ? z[i0 + 2] : -INFINITY;
+            }
+#pragma unroll
+            for (int u = 0; u < UN; ++u) {
+                const int64_t i0 = base + u * kStep + 2 * lane;
+                if (base + u * kStep >= end) break;  // warp-uniform
+                const double a = sanitize(v[u].x), c = sanitize(v[u].y);
+                const double up = __shfl_up_sync(0xffffffffu, c, 1), dn = __shfl_down_sync(0xffffffffu, a, 1);
+                const double l = lane == 0 ? sanitize(lft[u]) : up;
+                const double r = lane == 31 ? sanitize(rgt[u]) : dn;
+                L.offer(a, i0, i0 < K && a > l && a >= c);
+                L.offer(c, i0 + 1, i0 + 1 < K && c > a && c >= r);
+            }
         }
-        L.offer(v, i, peak);
+    } else {
+        for (int64_t base = begin + wid * 32; base < end; base += kTopkThreads) {
+            const int64_t i = base + lane;
+            bool peak = false;
+            double v = -INFINITY;
+            if (i < K) {
+                v = sanitize(z[i]);
+                const double l = i > 0 ? sanitize(z[i - 1]) : -INFINITY;
+                const double r = i + 1 < K ? sanitize(z[i + 1]) : -INFINITY;
+                peak = v > l && v >= r;
+            }
+            L.offer(v, i, peak);
+        }
     }
     cta_merge_and_write<SLOTS>(L, p, b, blockIdx.x, p.nblk == 1, sz, si);
 }

@@ -303,3 +303,23 @@ def test_topk_batched_matches_single(fr, oracle_mod):
     idx = fr.fredec_topk_batched(z, 5)
     for b in range(z.shape[0]):
         assert idx[b].tolist() == oracle_mod.topk(z[b], 5)[0].tolist()
+
+
+@pytest.mark.parametrize("K", [1, 2, 63, 64, 65, 511, 512, 513, 1024, 4099, 100_000])
+def test_topk_vector_path_edges(fr, oracle_mod, K):
+    """The 16-byte-load path (aligned rows) and the scalar path (odd K: every other row is
+    misaligned): peaks at tile, warp and CTA boundaries, NaN, ties and both grid edges."""
+    rng = np.random.Generator(np.random.PCG64(K))
+    B = 4
+    z = rng.integers(0, 6, (B, K)).astype(np.float64)            # many ties and plateaus
+    z[1] = rng.gamma(1.0, 3.0, K)
+    z[1, ::max(1, K // 7)] = np.nan
+    z[2, 0] = 100.0
+    z[2, -1] = 100.0
+    for e in (63, 64, 511, 512, 1023, 1024):                     # peaks exactly at boundaries
+        if e < K:
+            z[3, e] = 50.0 + e
+    k = min(K, 7)
+    idx = fr.fredec_topk_batched(z, k)
+    for b in range(B):
+        assert idx[b].tolist() == oracle_mod.topk(z[b], k)[0].tolist(), (K, b)
