@@ -193,6 +193,19 @@ int fredec_phase1(const double* t, const double* x, const double* w, int64_t N,
 int fredec_trig_averages(const double* t, const double* x, const double* w, int64_t N,
                          const double* freqs, int64_t M, double* out);
 
+/*
+ * fredec_subset_fits -- the linear multifrequency fit (section 3: Q = L L^T,
+ * a = L^{-1} g, l = D - |a|^2 with g, Q of eqs. 15-16; reading G2) for EVERY subset of a pool of n
+ * frequencies, as phase 2 needs them (2^n - 1 values), the frequencies held fixed
+ * (the l_m(f') of eq. 7, PAPER.md:81 -- not the locally refitted l_{m,loc}):
+ *   l_out[mask] = min over theta of <(x - theta_0 - sum_{j in mask} (a_j cos 2 pi f_j t + b_j sin 2 pi f_j t))^2>
+ * for mask = 0 .. 2^n - 1 (bit j selects freqs[j]); l_out[0] is the chi-square of the constant alone.
+ * A function that the preceding ones of its subset already span (equal frequencies) is dropped
+ * (rule S6).  t, x, w [N]; freqs [n], 1 <= n <= 25, N >= 2n + 2; l_out [2^n].
+ */
+int fredec_subset_fits(const double* t, const double* x, const double* w, int64_t N,
+                       const double* freqs, int32_t n, double* l_out);
+
 /* ----------------------------------------------------------------- runtime control */
 
 /* Stream on which all work is enqueued (a cudaStream_t passed as void*); NULL = default. */

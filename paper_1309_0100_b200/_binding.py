@@ -35,6 +35,7 @@ SIGNATURES = {
     "fredec_phase1": (C.c_int, [_P, _P, _P, _I64, _F64, _F64, _I64, _F64, _F64, _F64, _I32, _I32,
                                 _P, _P, _P, _I32, _P, C.POINTER(C.c_int32)]),
     "fredec_trig_averages": (C.c_int, [_P, _P, _P, _I64, _P, _I64, _P]),
+    "fredec_subset_fits": (C.c_int, [_P, _P, _P, _I64, _P, _I32, _P]),
     "fredec_set_stream": (C.c_int, [_P]),
     "fredec_last_timing": (C.c_int, [C.POINTER(C.c_double)]),
     "fredec_last_launches": (C.c_int, []),
@@ -260,6 +261,16 @@ def fredec_trig_averages(t, x, w, freqs, out=None):
     (pt, kt), (px, kx), (pw, kw), (pf, kf), (po, ko) = map(_ptr, (t, x, w, freqs, res))
     _check(lib().fredec_trig_averages(pt, px, pw, N, pf, M, po), "fredec_trig_averages")
     return res if out is None or ko is res else ko
+
+
+def fredec_subset_fits(t, x, w, freqs, l_out=None):
+    """l[mask] = min chi2 of constant + sinusoids at the frequencies selected by mask, for all
+    2^n subsets of freqs; see include/fredec.h."""
+    N, n = int(t.shape[-1]), int(freqs.shape[-1])
+    res = _empty_like_kind(t, (1 << n,)) if l_out is None else l_out
+    (pt, kt), (px, kx), (pw, kw), (pf, kf), (po, ko) = map(_ptr, (t, x, w, freqs, res))
+    _check(lib().fredec_subset_fits(pt, px, pw, N, pf, n, po), "fredec_subset_fits")
+    return res if l_out is None or ko is res else ko
 
 
 def fredec_last_timing() -> dict:

@@ -14,6 +14,7 @@
 #include "prep_kernel.cuh"
 #include "scan_mma_kernel.cuh"
 #include "stat_kernel.cuh"
+#include "subset_kernel.cuh"
 #include "trig_kernel.cuh"
 #include "topk_kernel.cuh"
 
@@ -78,7 +79,7 @@ struct State {
     cudaStream_t stream = nullptr;
     cudaEvent_t ev[kNumEvents] = {};
     DevBuf in_t, in_x, in_w, in_base, in_z, out_z, out_idx, out_chi2;
-    DevBuf p1_base, p1_freq, p1_z, p1_idx, p1_stats, tab, srec, psi, xt, info, ws, red, part_z, part_i, count, sink;
+    DevBuf gram, p1_base, p1_freq, p1_z, p1_idx, p1_stats, tab, srec, psi, xt, info, ws, red, part_z, part_i, count, sink;
     HostBuf h_info, h_count;
     int last_cuda = 0;
     double timing[4] = {0, 0, 0, 0};
@@ -676,6 +677,38 @@ int fredec_trig_averages(const double* t, const double* x, const double* w, int6
     return FREDEC_OK;
 }
 
+int fredec_subset_fits(const double* t, const double* x, const double* w, int64_t N, const double* freqs, int32_t n,
+                       double* l_out)
+{
+    if (!t || !x || !w || !freqs || !l_out || n < 1 || n > 25 || N < 2 * (int64_t)n + 2) return FREDEC_EINVAL;
+    int rc = begin_call();
+    if (rc) return rc;
+    cudaStream_t st = g.stream;
+    const int M = 2 * n + 1;
+    const size_t total = (size_t)1 << n;
+    const double *dt, *dx, *dw, *dfr;
+    if ((rc = stage_in(t, (size_t)N, g.in_t, &dt))) return rc;
+    if ((rc = stage_in(x, (size_t)N, g.in_x, &dx))) return rc;
+    if ((rc = stage_in(w, (size_t)N, g.in_w, &dw))) return rc;
+    if ((rc = stage_in(freqs, (size_t)n, g.p1_freq, &dfr))) return rc;
+    double *dl, *hl;
+    if ((rc = stage_out(l_out, total, g.out_z, &dl, &hl))) return rc;
+    CK(g.p1_base.reserve((size_t)M * N * 8));
+    CK(g.gram.reserve((size_t)(M + 1) * (M + 1) * 8));
+    CK(launch_sin_base(dt, N, dfr, n, g.p1_base.as<double>(), st));
+    CK(launch_gram(g.p1_base.as<double>(), dx, dw, N, M, g.gram.as<double>(), st));
+    CK(cudaEventRecord(g.ev[2], st));
+    CK(launch_subset_fits(g.gram.as<double>(), n, dl, g.sm_count, st));
+    CK(cudaEventRecord(g.ev[3], st));
+    g.launches += 3;
+    if (hl) CK(cudaMemcpyAsync(hl, dl, total * 8, cudaMemcpyDeviceToHost, st));
+    CK(cudaEventRecord(g.ev[6], st));
+    CK(cudaStreamSynchronize(st));
+    g.timing[1] = ev_ms(2, 3);
+    g.timing[3] = ev_ms(0, 6);
+    return FREDEC_OK;
+}
+
 int fredec_set_stream(void* cuda_stream)
 {
     g.stream = static_cast<cudaStream_t>(cuda_stream);
@@ -712,7 +745,7 @@ int fredec_fp64_peak(int64_t iters, double* tflops_out, double* ms_out)
 
 int fredec_shutdown(void)
 {
-    DevBuf* bufs[] = {&g.in_t, &g.in_x, &g.in_w, &g.in_base, &g.in_z, &g.out_z, &g.out_idx, &g.out_chi2, &g.p1_base, &g.p1_freq, &g.p1_z, &g.p1_idx, &g.p1_stats, &g.tab, &g.srec,
+    DevBuf* bufs[] = {&g.in_t, &g.in_x, &g.in_w, &g.in_base, &g.in_z, &g.out_z, &g.out_idx, &g.out_chi2, &g.gram, &g.p1_base, &g.p1_freq, &g.p1_z, &g.p1_idx, &g.p1_stats, &g.tab, &g.srec,
                       &g.psi,  &g.xt,   &g.info, &g.ws, &g.red,     &g.part_z, &g.part_i, &g.count, &g.sink};
     for (DevBuf* b : bufs) b->release();
     g.h_info.release();

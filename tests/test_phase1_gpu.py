@@ -127,3 +127,35 @@ def test_trig_averages_parity(fr, oracle_mod, N, M):
     assert np.all(np.abs(got - ref) <= 4 * N * np.finfo(float).eps * scale + 1e-300)
     gd = fr.fredec_trig_averages(*[torch.from_numpy(a).cuda() for a in (t, x, w, freqs)])
     assert np.array_equal(gd.cpu().numpy(), got)
+
+
+@pytest.mark.parametrize("n,N", [(1, 4), (3, 40), (6, 200), (10, 1000)])
+def test_subset_fits_parity(fr, p1, n, N):
+    """Every subset's linear fit.  Tolerance: l is a Schur complement of
+    numbers of size D = <x^2>, so errors are relative to D: 1e-10 D (conditioning of a pool with
+    well separated frequencies times a few hundred roundings)."""
+    import torch
+    rng = np.random.Generator(np.random.PCG64(77 * n + N))
+    t = np.sort(rng.uniform(0.0, 500.0, N))
+    freqs = np.sort(rng.uniform(0.01, 0.9, n))
+    x = rng.standard_normal(N) + sum(rng.uniform(0.5, 2.0) * np.sin(2 * np.pi * f * t + rng.uniform(0, 6))
+                                     for f in freqs[: max(1, n // 2)])
+    w = rng.uniform(0.5, 2.0, N)
+    ref = p1.subset_fits(t, x, w, freqs)
+    got = fr.fredec_subset_fits(t, x, w, freqs)
+    D = float(np.sum(w * x * x))
+    assert got.shape == ref.shape and np.all(np.abs(got - ref) <= 1e-10 * D)
+    gd = fr.fredec_subset_fits(*[torch.from_numpy(a).cuda() for a in (t, x, w, freqs)])
+    assert np.array_equal(gd.cpu().numpy(), got)
+
+
+def test_subset_fits_duplicate_frequency_and_errors(fr, p1):
+    t, x, w, _ = inputs.random_series(3, 60, 0)
+    freqs = np.array([0.2, 0.2, 0.31])
+    ref = p1.subset_fits(t, x, w, freqs)
+    got = fr.fredec_subset_fits(t, x, w, freqs)
+    assert np.all(np.isfinite(got)) and np.all(np.abs(got - ref) <= 1e-9 * ref[0])
+    with pytest.raises(fr.FredecError):
+        fr.fredec_subset_fits(t, x, w, np.linspace(0.1, 0.9, 26))           # n > 25
+    with pytest.raises(fr.FredecError):
+        fr.fredec_subset_fits(t[:5], x[:5], w[:5], np.array([0.1, 0.2]))    # N < 2n + 2
