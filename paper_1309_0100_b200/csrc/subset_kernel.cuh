@@ -13,7 +13,8 @@ cudaError_t launch_gram(const double* basis, const double* x, const double* w, i
                         cudaStream_t stream);
 
 // l_out[mask] = D - |L^{-1} g|^2 for the sub-model {1} + {cos, sin of frequency j : bit j of mask},
-// mask = 0 .. 2^n - 1.  One warp per subset, matrices in shared memory.
+// mask = 0 .. 2^n - 1.  Depth-first over the subsets, one warp per subtree, factor rows
+// in shared memory.
 cudaError_t launch_subset_fits(const double* A, int n, double* l_out, int sm_count, cudaStream_t stream);
 
 }  // namespace fredec

@@ -149,6 +149,24 @@ def test_subset_fits_parity(fr, p1, n, N):
     assert np.array_equal(gd.cpu().numpy(), got)
 
 
+@pytest.mark.parametrize("n", [13, 17])
+def test_subset_fits_large_pool_sampled(fr, p1, n):
+    """Pools beyond one depth-first task (n > 11: a prefix of n - 6 frequencies per warp, then a walk
+    over 64 extensions): sampled subsets, the empty and the full one, against the oracle."""
+    rng = np.random.Generator(np.random.PCG64(n))
+    N = 600
+    t = np.sort(rng.uniform(0.0, 800.0, N))
+    freqs = np.sort(rng.uniform(0.01, 0.9, n))
+    x = rng.standard_normal(N) + sum(1.5 * np.cos(2 * np.pi * f * t + j) for j, f in enumerate(freqs[::3]))
+    w = rng.uniform(0.5, 2.0, N)
+    got = fr.fredec_subset_fits(t, x, w, freqs)
+    masks = np.unique(np.concatenate([[0, (1 << n) - 1, 1, 1 << (n - 1)], rng.integers(0, 1 << n, 300)]))
+    ref = p1.subset_fits(t, x, w, freqs, masks=masks)
+    D = float(np.sum(w * x * x))
+    assert np.all(np.abs(got[masks] - ref) <= 1e-10 * D)
+    assert np.all(got >= 0.0) and np.all(got <= got[0] * (1 + 1e-12))
+
+
 def test_subset_fits_duplicate_frequency_and_errors(fr, p1):
     t, x, w, _ = inputs.random_series(3, 60, 0)
     freqs = np.array([0.2, 0.2, 0.31])
