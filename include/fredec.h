@@ -206,6 +206,24 @@ int fredec_trig_averages(const double* t, const double* x, const double* w, int6
 int fredec_subset_fits(const double* t, const double* x, const double* w, int64_t N,
                        const double* freqs, int32_t n, double* l_out);
 
+/*
+ * fredec_refine -- the local multifrequency fit l_{n,loc} (section 3, eq. 17): starting
+ * from preliminary frequencies (periodogram peaks), iterate { exact linear fit of theta (eq. 14) ->
+ * quadratic model of chi2 in (theta, f) with g_f, Q_f (their theta-part vanishes / equals Q) -> step
+ * Q_f^{-1} g_f -> update f }, and finish with one more linear fit.  Model: eq. 2, constant +
+ * n sinusoids; times are centred on their weighted mean.  Q_f is the Gauss-Newton
+ * (Fisher) matrix <J J^T>, J = (model functions, d mu / d f_k).  Readings (R1-R2):
+ * a frequency step is clamped to +-0.5 / T_eff so that the fit stays inside its periodogram peak
+ * ("local"); iteration stops when max_k |step_k| * T_eff <= tol.
+ *   t, x, w [N];  freqs [n] in: start, out: refined (host or device);  1 <= n <= 25, N >= 3n + 2
+ *   max_iter >= 0 frequency updates at most;  tol > 0 (cycles of phase drift over T_eff)
+ *   l_out      HOST double: min chi2 at the returned frequencies;  iters_out  HOST int32 (may be NULL)
+ * Returns FREDEC_OK, or FREDEC_ESINGULAR when the normal equations are singular (equal frequencies).
+ */
+int fredec_refine(const double* t, const double* x, const double* w, int64_t N,
+                  double* freqs, int32_t n, int32_t max_iter, double tol,
+                  double* l_out, int32_t* iters_out);
+
 /* ----------------------------------------------------------------- runtime control */
 
 /* Stream on which all work is enqueued (a cudaStream_t passed as void*); NULL = default. */

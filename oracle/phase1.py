@@ -133,3 +133,51 @@ def subset_fits(t, x, w, freqs, tau: float = 1e-10, masks=None):
                 a[i] = (g[idx[i]] - L[i, :i] @ a[:i]) / L[i, i]
         out[pos] = max(D - a @ a, 0.0)
     return out
+
+
+def refine(t, x, w, freqs, max_iter: int = 20, tol: float = 1e-9):
+    """PAPER.md:177-185 (section 3, eq. 17): the local multifrequency fit.  Each iteration: exact linear
+    fit of theta at the current frequencies (eq. 14: Q = L L^T, a = L^{-1} g, theta = L^{-T} a), then the
+    quadratic model of chi2 in xi = (theta, f) around (theta*, f): gradient g_f = <(x - mu) J> (its theta
+    part is zero), matrix Q_f = <J J^T> with J = (model functions, d mu/d f_k) (its leading block is Q),
+    step Q_f^{-1} g_f, frequencies updated; a last linear fit gives l_{n,loc}.  Times centred on their
+    weighted mean.  Readings R1, R2: |step| <= 0.5 / T_eff; stop when
+    max |step| T_eff <= tol.  Returns (freqs, l, iterations)."""
+    t, x, w = (np.asarray(a, dtype=np.float64) for a in (t, x, w))
+    f = np.array(freqs, dtype=np.float64, copy=True)
+    n = f.size
+    t0 = np.sum(w * t) / np.sum(w)
+    tc = t - t0
+    T_eff, _ = bandwidth(t, w, 1.0)
+    D = np.sum(w * x * x)
+    iters, converged = 0, max_iter == 0
+    while True:
+        Phi = sinusoid_base(tc, f)
+        Q = (Phi * w) @ Phi.T
+        g = (Phi * w) @ x
+        L = np.linalg.cholesky(Q)
+        a = _forward(L, g)
+        theta = _forward(L.T[::-1, ::-1], a[::-1])[::-1]          # back substitution
+        l = D - a @ a
+        if converged or iters == max_iter:
+            return f, max(float(l), 0.0), iters
+        dmu = np.stack([2.0 * np.pi * tc * (-theta[2 * k + 1] * Phi[2 * k + 2] + theta[2 * k + 2] * Phi[2 * k + 1])
+                        for k in range(n)])
+        J = np.vstack([Phi, dmu])
+        Qf = (J * w) @ J.T
+        gf = (J * w) @ (x - theta @ Phi)
+        Lf = np.linalg.cholesky(Qf)
+        af = _forward(Lf, gf)
+        step = _forward(Lf.T[::-1, ::-1], af[::-1])[::-1]
+        df = np.clip(step[2 * n + 1:], -0.5 / T_eff, 0.5 / T_eff)
+        f = f + df
+        iters += 1
+        converged = np.max(np.abs(df)) * T_eff <= tol
+
+
+def _forward(L, b):
+    """Solves L y = b for lower-triangular L by forward substitution."""
+    y = np.zeros_like(b, dtype=np.float64)
+    for i in range(b.size):
+        y[i] = (b[i] - L[i, :i] @ y[:i]) / L[i, i]
+    return y

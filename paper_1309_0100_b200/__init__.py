@@ -9,5 +9,5 @@ from ._binding import (  # noqa: F401
     fredec_chi2_base, fredec_chi2_base_batched, fredec_fp64_peak, fredec_last_launches,
     fredec_last_timing, fredec_scan, fredec_scan_batched, fredec_scan_topk, fredec_scan_topk_batched, fredec_set_stream, fredec_shutdown,
     fredec_topk, fredec_topk_batched, fredec_version, lib,
-    fredec_bandwidth, fredec_fap1, fredec_phase1, fredec_subset_fits, fredec_trig_averages, fredec_zstat,
+    fredec_bandwidth, fredec_fap1, fredec_phase1, fredec_refine, fredec_subset_fits, fredec_trig_averages, fredec_zstat,
 )

@@ -36,6 +36,8 @@ SIGNATURES = {
                                 _P, _P, _P, _I32, _P, C.POINTER(C.c_int32)]),
     "fredec_trig_averages": (C.c_int, [_P, _P, _P, _I64, _P, _I64, _P]),
     "fredec_subset_fits": (C.c_int, [_P, _P, _P, _I64, _P, _I32, _P]),
+    "fredec_refine": (C.c_int, [_P, _P, _P, _I64, _P, _I32, _I32, _F64, C.POINTER(C.c_double),
+                                C.POINTER(C.c_int32)]),
     "fredec_set_stream": (C.c_int, [_P]),
     "fredec_last_timing": (C.c_int, [C.POINTER(C.c_double)]),
     "fredec_last_launches": (C.c_int, []),
@@ -271,6 +273,17 @@ def fredec_subset_fits(t, x, w, freqs, l_out=None):
     (pt, kt), (px, kx), (pw, kw), (pf, kf), (po, ko) = map(_ptr, (t, x, w, freqs, res))
     _check(lib().fredec_subset_fits(pt, px, pw, N, pf, n, po), "fredec_subset_fits")
     return res if l_out is None or ko is res else ko
+
+
+def fredec_refine(t, x, w, freqs, max_iter=20, tol=1e-9):
+    """Local multifrequency fit: returns (refined freqs [n] as numpy, l = min chi2, iterations)."""
+    N = int(t.shape[-1])
+    f = np.array(freqs.cpu().numpy() if _is_torch(freqs) else freqs, dtype=np.float64, copy=True)
+    l, it = C.c_double(), C.c_int32()
+    (pt, kt), (px, kx), (pw, kw) = map(_ptr, (t, x, w))
+    _check(lib().fredec_refine(pt, px, pw, N, f.ctypes.data, int(f.shape[0]), int(max_iter), float(tol),
+                               C.byref(l), C.byref(it)), "fredec_refine")
+    return f, l.value, it.value
 
 
 def fredec_last_timing() -> dict:

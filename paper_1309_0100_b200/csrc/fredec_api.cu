@@ -13,6 +13,7 @@
 #include "peak_kernel.cuh"
 #include "prep_kernel.cuh"
 #include "scan_mma_kernel.cuh"
+#include "refine_kernel.cuh"
 #include "stat_kernel.cuh"
 #include "subset_kernel.cuh"
 #include "trig_kernel.cuh"
@@ -79,7 +80,7 @@ struct State {
     cudaStream_t stream = nullptr;
     cudaEvent_t ev[kNumEvents] = {};
     DevBuf in_t, in_x, in_w, in_base, in_z, out_z, out_idx, out_chi2;
-    DevBuf gram, p1_base, p1_freq, p1_z, p1_idx, p1_stats, tab, srec, psi, xt, info, ws, red, part_z, part_i, count, sink;
+    DevBuf gram, rf, p1_base, p1_freq, p1_z, p1_idx, p1_stats, tab, srec, psi, xt, info, ws, red, part_z, part_i, count, sink;
     HostBuf h_info, h_count;
     int last_cuda = 0;
     double timing[4] = {0, 0, 0, 0};
@@ -709,6 +710,72 @@ int fredec_subset_fits(const double* t, const double* x, const double* w, int64_
     return FREDEC_OK;
 }
 
+int fredec_refine(const double* t, const double* x, const double* w, int64_t N, double* freqs, int32_t n,
+                  int32_t max_iter, double tol, double* l_out, int32_t* iters_out)
+{
+    if (!t || !x || !w || !freqs || !l_out || n < 1 || n > 25 || N < 3 * (int64_t)n + 2) return FREDEC_EINVAL;
+    if (max_iter < 0 || !(tol > 0.0) || on_device(l_out) || (iters_out && on_device(iters_out))) return FREDEC_EINVAL;
+    int rc = begin_call();
+    if (rc) return rc;
+    cudaStream_t st = g.stream;
+    const double *dt, *dx, *dw;
+    if ((rc = stage_in(t, (size_t)N, g.in_t, &dt))) return rc;
+    if ((rc = stage_in(x, (size_t)N, g.in_x, &dx))) return rc;
+    if ((rc = stage_in(w, (size_t)N, g.in_w, &dw))) return rc;
+    double bw[4];
+    if ((rc = device_bandwidth(dt, dw, N, bw))) return rc;
+    const double T_eff = bw[0], t0 = bw[2];
+    if (!(T_eff > 0.0)) return FREDEC_EDATA;
+    const int lin = 2 * n + 1, full = 3 * n + 1;
+    CK(g.p1_base.reserve((size_t)full * N * 8));
+    CK(g.p1_freq.reserve((size_t)n * 8));
+    CK(g.gram.reserve((size_t)(full + 1) * (full + 1) * 8));
+    CK(g.rf.reserve((size_t)(full + n + 4) * 8));
+    double* dfreq = g.p1_freq.as<double>();
+    double* rows = g.p1_base.as<double>();
+    double* theta = g.rf.as<double>();   // [full]
+    double* dstep = theta + full;        // [n]
+    double* out2 = dstep + n;            // [2] linear fit, [2] Gauss-Newton step
+    const bool freqs_dev = on_device(freqs);
+    CK(cudaMemcpyAsync(dfreq, freqs, (size_t)n * 8, freqs_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+    std::vector<double> hstep((size_t)n);
+    double hout[4];
+    int iters = 0, launches = 1;
+    bool converged = max_iter == 0;
+    while (true) {
+        // linear fit at the current frequencies (eq. 14)
+        CK(launch_model_rows(dt, N, t0, dfreq, n, nullptr, rows, st));
+        CK(launch_gram(rows, dx, dw, N, lin, g.gram.as<double>(), st));
+        CK(launch_chol_solve(g.gram.as<double>(), lin, theta, out2, st));
+        launches += 3;
+        if (converged || iters == max_iter) break;
+        // quadratic model in (theta, f) and its step (eq. 17)
+        CK(launch_model_rows(dt, N, t0, dfreq, n, theta, rows, st));
+        CK(launch_gram(rows, dx, dw, N, full, g.gram.as<double>(), st));
+        CK(launch_gn_step(g.gram.as<double>(), n, theta, 0.5 / T_eff, dstep, out2 + 2, st));
+        CK(launch_axpy_small(dfreq, dstep, n, st));
+        launches += 4;
+        CK(cudaMemcpyAsync(hstep.data(), dstep, (size_t)n * 8, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(hout, out2, 32, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        if (hout[1] != 0.0 || hout[3] != 0.0) return FREDEC_ESINGULAR;
+        ++iters;
+        double worst = 0.0;
+        for (int k = 0; k < n; ++k) worst = std::fmax(worst, std::fabs(hstep[k]));
+        converged = worst * T_eff <= tol;
+    }
+    CK(cudaMemcpyAsync(hout, out2, 16, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(freqs, dfreq, (size_t)n * 8, freqs_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
+    CK(cudaEventRecord(g.ev[6], st));
+    CK(cudaStreamSynchronize(st));
+    g.timing[3] = ev_ms(0, 6);
+    g.launches = launches;
+    if (hout[1] != 0.0) return FREDEC_ESINGULAR;
+    *l_out = hout[0];
+    if (iters_out) *iters_out = iters;
+    return FREDEC_OK;
+}
+
 int fredec_set_stream(void* cuda_stream)
 {
     g.stream = static_cast<cudaStream_t>(cuda_stream);
@@ -745,7 +812,7 @@ int fredec_fp64_peak(int64_t iters, double* tflops_out, double* ms_out)
 
 int fredec_shutdown(void)
 {
-    DevBuf* bufs[] = {&g.in_t, &g.in_x, &g.in_w, &g.in_base, &g.in_z, &g.out_z, &g.out_idx, &g.out_chi2, &g.gram, &g.p1_base, &g.p1_freq, &g.p1_z, &g.p1_idx, &g.p1_stats, &g.tab, &g.srec,
+    DevBuf* bufs[] = {&g.in_t, &g.in_x, &g.in_w, &g.in_base, &g.in_z, &g.out_z, &g.out_idx, &g.out_chi2, &g.gram, &g.rf, &g.p1_base, &g.p1_freq, &g.p1_z, &g.p1_idx, &g.p1_stats, &g.tab, &g.srec,
                       &g.psi,  &g.xt,   &g.info, &g.ws, &g.red,     &g.part_z, &g.part_i, &g.count, &g.sink};
     for (DevBuf* b : bufs) b->release();
     g.h_info.release();

@@ -177,3 +177,46 @@ def test_subset_fits_duplicate_frequency_and_errors(fr, p1):
         fr.fredec_subset_fits(t, x, w, np.linspace(0.1, 0.9, 26))           # n > 25
     with pytest.raises(fr.FredecError):
         fr.fredec_subset_fits(t[:5], x[:5], w[:5], np.array([0.1, 0.2]))    # N < 2n + 2
+
+
+@pytest.mark.parametrize("noise,n", [(0.0, 2), (0.3, 2), (0.5, 4)])
+def test_refine_parity(fr, p1, noise, n):
+    """Local multifrequency fit.  Both sides stop on the same criterion
+    (max |step| T_eff <= tol), so the frequencies agree to a few tol / T_eff and l to rounding of a
+    Schur complement of size D: 1e-9 D (the iteration count may differ by one at the threshold)."""
+    rng = np.random.Generator(np.random.PCG64(90 + n))
+    N = 400
+    t = np.sort(rng.uniform(50.0, 650.0, N))
+    f_true = np.sort(rng.uniform(0.02, 0.4, n))
+    x = 0.3 + sum((2.5 - 0.4 * k) * np.cos(2 * np.pi * f * t + k) for k, f in enumerate(f_true)) \
+        + noise * rng.standard_normal(N)
+    w = rng.uniform(0.5, 2.0, N)
+    T = t.max() - t.min()
+    start = f_true + rng.uniform(-0.25, 0.25, n) / T
+    tol = 1e-9
+    f_ref, l_ref, it_ref = p1.refine(t, x, w, start, max_iter=30, tol=tol)
+    f, l, it = fr.fredec_refine(t, x, w, start, max_iter=30, tol=tol)
+    T_eff, _ = p1.bandwidth(t, w, 1.0)
+    D = float(np.sum(w * x * x))
+    assert np.max(np.abs(f - f_ref)) * T_eff <= 10 * tol
+    assert abs(l - l_ref) <= 1e-9 * D and abs(it - it_ref) <= 1
+    if noise == 0.0:
+        assert np.max(np.abs(f - f_true)) * T < 1e-7 and l <= 1e-12 * D
+    # device pointers; and no iterations = the linear fit at the start
+    import torch
+    fd, ld, _ = fr.fredec_refine(*[torch.from_numpy(a).cuda() for a in (t, x, w)], start, max_iter=30, tol=tol)
+    assert np.array_equal(fd, f) and ld == l
+    f0, l0, it0 = fr.fredec_refine(t, x, w, start, max_iter=0)
+    _, l0_ref, _ = p1.refine(t, x, w, start, max_iter=0)
+    assert it0 == 0 and np.array_equal(f0, start) and abs(l0 - l0_ref) <= 1e-9 * D
+
+
+def test_refine_errors(fr):
+    t, x, w, _ = inputs.random_series(2, 60, 0)
+    with pytest.raises(fr.FredecError) as e:
+        fr.fredec_refine(t, x, w, np.array([0.2, 0.2]))           # equal frequencies: singular
+    assert e.value.code == fr.FREDEC_ESINGULAR
+    with pytest.raises(fr.FredecError):
+        fr.fredec_refine(t[:7], x[:7], w[:7], np.array([0.1, 0.2]))   # N < 3n + 2
+    with pytest.raises(fr.FredecError):
+        fr.fredec_refine(t, x, w, np.array([0.1]), tol=0.0)
