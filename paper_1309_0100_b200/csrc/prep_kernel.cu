@@ -181,9 +181,10 @@ __global__ void __launch_bounds__(kTableThreads) table_kernel(TableParams p)
                 const int j = pass * p.NB + (f - 1);
                 m = (j < p.d && real) ? wi * psi[(int64_t)j * N + i] : 0.0;
             }
-            double* tile = grp + (f * NT + nt) * 32;
-            tile[n0 * 4 + k] = m * c;
-            tile[(n0 + 1) * 4 + k] = m * s;
+            // column tiles are stored in pairs (one 16-byte load per lane fetches the fragments of two)
+            double* tile = grp + (f * (NT / 2) + nt / 2) * 64 + (nt & 1);
+            tile[(n0 * 4 + k) * 2] = m * c;
+            tile[((n0 + 1) * 4 + k) * 2] = m * s;
         }
     }
 }

@@ -201,7 +201,7 @@ __device__ __forceinline__ void round_mma(Tiles<H, NOCT, NB>& acc, RingPos& rp, 
                                           uint64_t* bar_done)
 {
     constexpr int NT = H / 4, NF = NB + 2, GROUP = NF * NT * 32, CAP = kNW * NOCT;
-    const double* tk = nullptr;
+    const double2* tk = nullptr;  // this lane's table fragments (pairs of column tiles)
     const double2* sk = nullptr;
     int ksl = 0;
     int nslot = 0;
@@ -214,7 +214,7 @@ __device__ __forceinline__ void round_mma(Tiles<H, NOCT, NB>& acc, RingPos& rp, 
                 mbar_wait(&bar_seed[rp.slot], rp.par);
             }
             const unsigned char* base = smem + rp.slot * slot_bytes;
-            tk = reinterpret_cast<const double*>(base) + lane;
+            tk = reinterpret_cast<const double2*>(base) + lane;
             sk = reinterpret_cast<const double2*>(base + tab_bytes) + (size_t)role.off * 32 + lane;
             nslot = rp.slot + 1;
             npar = rp.par;
@@ -236,22 +236,27 @@ __device__ __forceinline__ void round_mma(Tiles<H, NOCT, NB>& acc, RingPos& rp, 
 #pragma unroll
             for (int f = 0; f < NF; ++f) {
 #pragma unroll
-                for (int t = 0; t < NT; ++t) {
-                    const double bf = tk[(f * NT + t) * 32];
+                for (int tp = 0; tp < NT / 2; ++tp) {
+                    const double2 b2 = tk[(f * (NT / 2) + tp) * 32];
 #pragma unroll
-                    for (int o = 0; o < CNT; ++o) {
-                        if (f < NF - 1) {
-                            FREDEC_DMMA(acc.v[o][0][f][t], a[o].x, bf);
-                            FREDEC_DMMA(acc.v[o][1][f][t], a[o].y, bf);
-                        } else {
-                            FREDEC_DMMA(acc.v[o][0][f][t], c2[o], bf);
-                            FREDEC_DMMA(acc.v[o][1][f][t], s2[o], bf);
+                    for (int h2 = 0; h2 < 2; ++h2) {
+                        const int t = 2 * tp + h2;
+                        const double bf = h2 == 0 ? b2.x : b2.y;
+#pragma unroll
+                        for (int o = 0; o < CNT; ++o) {
+                            if (f < NF - 1) {
+                                FREDEC_DMMA(acc.v[o][0][f][t], a[o].x, bf);
+                                FREDEC_DMMA(acc.v[o][1][f][t], a[o].y, bf);
+                            } else {
+                                FREDEC_DMMA(acc.v[o][0][f][t], c2[o], bf);
+                                FREDEC_DMMA(acc.v[o][1][f][t], s2[o], bf);
+                            }
                         }
                     }
                 }
             }
         }
-        tk += GROUP;
+        tk += GROUP / 2;
         sk += CAP * 32;
         ++ksl;
         if (ksl == KS - 1 || KS == 1) {  // one group before the end: is the next slot there already?

@@ -12,12 +12,12 @@ namespace fredec {
 // phi_i +- alpha_hi with phi_i = 2 pi f_c t'_i (depends on the run: a "seed") and
 // alpha_hi = 2 pi (h - 1/2) df t'_i (the same for every run: a per-observation TABLE).
 //
-// Table, per group of 4 observations: [family][column tile][32 doubles in B-fragment order],
+// Table, per group of 4 observations: [family][column tile pair][32 lanes in B-fragment order][2 tiles],
 // families: 0 = y (w x~), 1..NB = p_j (w psi_j), NB+1 = w/2.  Column n = 2 hh + type of tile
 // nt belongs to h = 4 nt + hh + 1; type 0 = cos, 1 = sin of alpha_h (of 2 alpha_h in the
 // w family); the entry is multiplier x trig value.  Fragment order: element (k = observation
-// within the group, n = column) sits at n * 4 + k, i.e. at the lane that owns it in
-// mma.m8n8k4's B operand.
+// within the group, n = column) belongs to lane n * 4 + k, the lane that owns it in mma.m8n8k4's
+// B operand; the lane's entries of tiles 2p and 2p+1 are adjacent (one LDS.128).  H % 8 == 0.
 __host__ __device__ constexpr int mma_nt(int H) { return H / 4; }
 __host__ __device__ constexpr int mma_nf(int NB) { return NB + 2; }
 __host__ __device__ constexpr int mma_group_doubles(int H, int NB) { return mma_nf(NB) * mma_nt(H) * 32; }
