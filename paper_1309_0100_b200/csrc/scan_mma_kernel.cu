@@ -191,84 +191,97 @@ struct RingPos {
     bool ready;
 };
 
-// a6 for one round: all tiles of the series, CNT = units this warp owns in the round.  One flat
-// loop over the groups of 4 observations; the ring slot changes every KS groups without leaving
-// the loop, so the MMA stream continues across slots.
+// a6 for one group of 4 observations: A fragments (seeds), B fragments (table), 2 * NF * NT MMAs per unit.
+template <int CNT, int H, int NOCT, int NB>
+__device__ __forceinline__ void mma_group(Tiles<H, NOCT, NB>& acc, const double2* tk, const double2* sk)
+{
+    constexpr int NT = H / 4, NF = NB + 2;
+    double2 a[CNT];
+    double c2[CNT], s2[CNT];
+#pragma unroll
+    for (int o = 0; o < CNT; ++o) {
+        a[o] = sk[o * 32];
+        c2[o] = fma(a[o].x, a[o].x, -(a[o].y * a[o].y));  // cos 2 phi
+        s2[o] = (a[o].x + a[o].x) * a[o].y;              // sin 2 phi
+    }
+#pragma unroll
+    for (int f = 0; f < NF; ++f) {
+#pragma unroll
+        for (int tp = 0; tp < NT / 2; ++tp) {
+            const double2 b2 = tk[(f * (NT / 2) + tp) * 32];
+#pragma unroll
+            for (int h2 = 0; h2 < 2; ++h2) {
+                const int t = 2 * tp + h2;
+                const double bf = h2 == 0 ? b2.x : b2.y;
+#pragma unroll
+                for (int o = 0; o < CNT; ++o) {
+                    if (f < NF - 1) {
+                        FREDEC_DMMA(acc.v[o][0][f][t], a[o].x, bf);
+                        FREDEC_DMMA(acc.v[o][1][f][t], a[o].y, bf);
+                    } else {
+                        FREDEC_DMMA(acc.v[o][0][f][t], c2[o], bf);
+                        FREDEC_DMMA(acc.v[o][1][f][t], s2[o], bf);
+                    }
+                }
+            }
+        }
+    }
+}
+
+// a6 for one round: all tiles of the series, CNT = units this warp owns in the round.  The ring slot
+// changes every KS groups; the next slot's barriers are looked at before the slot's last groups so
+// that the MMA stream continues across slots.
 template <int CNT, int H, int NOCT, int NB>
 __device__ __forceinline__ void round_mma(Tiles<H, NOCT, NB>& acc, RingPos& rp, const unsigned char* smem,
                                           size_t slot_bytes, size_t tab_bytes, int NS, int KS, int64_t G4,
                                           WarpRole role, int lane, uint64_t* bar_tab, uint64_t* bar_seed,
                                           uint64_t* bar_done)
 {
-    constexpr int NT = H / 4, NF = NB + 2, GROUP = NF * NT * 32, CAP = kNW * NOCT;
-    const double2* tk = nullptr;  // this lane's table fragments (pairs of column tiles)
-    const double2* sk = nullptr;
-    int ksl = 0;
-    int nslot = 0;
-    uint32_t npar = 0;
+    constexpr int NT = H / 4, NF = NB + 2, GROUP2 = NF * NT * 16, CAP = kNW * NOCT;  // GROUP2: double2 per group
 #pragma unroll 1
-    for (int64_t g = 0; g < G4; ++g) {
-        if (ksl == 0) {  // enter the slot
-            if (!rp.ready) {
-                mbar_wait(&bar_tab[rp.slot], rp.par);
-                mbar_wait(&bar_seed[rp.slot], rp.par);
-            }
-            const unsigned char* base = smem + rp.slot * slot_bytes;
-            tk = reinterpret_cast<const double2*>(base) + lane;
-            sk = reinterpret_cast<const double2*>(base + tab_bytes) + (size_t)role.off * 32 + lane;
-            nslot = rp.slot + 1;
-            npar = rp.par;
-            if (nslot == NS) {
-                nslot = 0;
-                npar ^= 1u;
-            }
-            rp.ready = false;
+    for (int64_t g = 0; g < G4; g += KS) {
+        const int ngrp = (int)min((int64_t)KS, G4 - g);
+        if (!rp.ready) {
+            mbar_wait(&bar_tab[rp.slot], rp.par);
+            mbar_wait(&bar_seed[rp.slot], rp.par);
         }
-        if (CNT > 0 && (ksl & (role.S - 1)) == role.sp) {
-            double2 a[CNT > 0 ? CNT : 1];
-            double c2[CNT > 0 ? CNT : 1], s2[CNT > 0 ? CNT : 1];
-#pragma unroll
-            for (int o = 0; o < CNT; ++o) {
-                a[o] = sk[o * 32];
-                c2[o] = fma(a[o].x, a[o].x, -(a[o].y * a[o].y));  // cos 2 phi
-                s2[o] = (a[o].x + a[o].x) * a[o].y;              // sin 2 phi
-            }
-#pragma unroll
-            for (int f = 0; f < NF; ++f) {
-#pragma unroll
-                for (int tp = 0; tp < NT / 2; ++tp) {
-                    const double2 b2 = tk[(f * (NT / 2) + tp) * 32];
-#pragma unroll
-                    for (int h2 = 0; h2 < 2; ++h2) {
-                        const int t = 2 * tp + h2;
-                        const double bf = h2 == 0 ? b2.x : b2.y;
-#pragma unroll
-                        for (int o = 0; o < CNT; ++o) {
-                            if (f < NF - 1) {
-                                FREDEC_DMMA(acc.v[o][0][f][t], a[o].x, bf);
-                                FREDEC_DMMA(acc.v[o][1][f][t], a[o].y, bf);
-                            } else {
-                                FREDEC_DMMA(acc.v[o][0][f][t], c2[o], bf);
-                                FREDEC_DMMA(acc.v[o][1][f][t], s2[o], bf);
-                            }
-                        }
-                    }
-                }
-            }
+        const unsigned char* base = smem + rp.slot * slot_bytes;
+        const double2* tk = reinterpret_cast<const double2*>(base) + lane;  // this lane's table fragments
+        const double2* sk = reinterpret_cast<const double2*>(base + tab_bytes) + (size_t)role.off * 32 + lane;
+        int nslot = rp.slot + 1;
+        uint32_t npar = rp.par;
+        if (nslot == NS) {
+            nslot = 0;
+            npar ^= 1u;
         }
-        tk += GROUP / 2;
-        sk += CAP * 32;
-        ++ksl;
-        if (ksl == KS - 1 || KS == 1) {  // one group before the end: is the next slot there already?
+        if (role.S == 1) {
+            // all but the last two groups, the look at the next slot, the last two groups
+            const int head = ngrp > 2 ? (ngrp - 2) & ~1 : 0;
+#pragma unroll 1
+            for (int ks = 0; ks < head; ks += 2) {
+                mma_group<CNT>(acc, tk, sk);
+                mma_group<CNT>(acc, tk + GROUP2, sk + CAP * 32);
+                tk += 2 * GROUP2;
+                sk += 2 * CAP * 32;
+            }
             rp.ready = mbar_test(&bar_tab[nslot], npar) & mbar_test(&bar_seed[nslot], npar);
+#pragma unroll 1
+            for (int ks = head; ks < ngrp; ++ks) {
+                mma_group<CNT>(acc, tk, sk);
+                tk += GROUP2;
+                sk += CAP * 32;
+            }
+        } else {
+            // a8: the S warps of a unit take the slot's groups in turn
+            rp.ready = false;
+#pragma unroll 1
+            for (int ks = role.sp; ks < ngrp; ks += role.S)
+                mma_group<CNT>(acc, tk + (size_t)ks * GROUP2, sk + (size_t)ks * CAP * 32);
         }
-        if (ksl == KS || g + 1 == G4) {  // leave the slot
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&bar_done[rp.slot]);
-            rp.slot = nslot;
-            rp.par = npar;
-            ksl = 0;
-        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bar_done[rp.slot]);
+        rp.slot = nslot;
+        rp.par = npar;
     }
 }
 
