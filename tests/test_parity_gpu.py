@@ -323,3 +323,19 @@ def test_topk_vector_path_edges(fr, oracle_mod, K):
     idx = fr.fredec_topk_batched(z, k)
     for b in range(B):
         assert idx[b].tolist() == oracle_mod.topk(z[b], k)[0].tolist(), (K, b)
+
+
+def test_long_series_many_ring_laps(fr, oracle_mod):
+    """N = 60 000 observations: ~1900 ring slots per round (hundreds of laps of the mbarrier ring),
+    a short grid so that every round is an observation-split round."""
+    rng = np.random.Generator(np.random.PCG64(60))
+    N, K = 60_000, 700
+    t = np.sort(rng.uniform(0.0, 5000.0, N))
+    x = 0.8 * np.sin(2 * np.pi * 0.0371 * t) + rng.standard_normal(N)
+    w = rng.uniform(0.5, 2.0, N)
+    base = inputs.base_offset_trend(t)
+    f0, df = 0.001, 1.1e-4
+    z_ref = oracle_mod.scan(t, x, w, base, f0, df, K, threads=0)
+    z = gpu_scan(fr, t, x, w, base, f0, df, K)
+    assert_parity(z, z_ref, "long series")
+    assert abs((f0 + df * int(np.argmax(z))) - 0.0371) < 2 * df
