@@ -40,7 +40,7 @@ WORKLOAD = "config4 survey: N=10000 obs x K=2000000 freqs, d=2 (offset+trend), t
 # FP64 roofline denominators: 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz
 FP64_LANES_PER_SM = 64
 L2_FLUSH_BYTES = 256 << 20
-ORACLE_SAMPLE_K = 20_000          # grid points of config 4 the CPU legs time per step
+ORACLE_SAMPLE_K = 100_000         # grid points of config 4 the CPU legs time per step (~20 core-seconds)
 # dram__bytes_read.sum + dram__bytes_write.sum of one scan_mma_kernel launch on config 4, from the
 # `ncu --set full` capture summarised in profiles/r1_scan_mma_kernel_ncu.md (read only: the 16 MB
 # periodogram is still in L2 when the kernel ends).  Algorithmic bytes: 10.6 MB table + 16 MB z.
