@@ -17,9 +17,11 @@ namespace fredec {
 
 namespace {
 
-constexpr int kPrepThreads = 256;
+constexpr int kPrepThreadsMax = 1024;  // one long series: as many threads as a CTA can have
+constexpr int kPrepThreadsMin = 256;   // many short series: several CTAs per SM
 
 // Fixed-order block sum, result broadcast to all threads.  `red` = 32 doubles of smem.
+template <int TH>
 __device__ double block_sum(double v, double* red)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -28,12 +30,13 @@ __device__ double block_sum(double v, double* red)
     __syncthreads();  // protect `red` from the previous call's readers
     if (lane == 0) red[wid] = v;
     __syncthreads();
-    double r = (lane < (kPrepThreads >> 5)) ? red[lane] : 0.0;
+    double r = (lane < (TH >> 5)) ? red[lane] : 0.0;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) r += __shfl_xor_sync(0xffffffffu, r, o);
     return r;
 }
 
+template <int TH>
 __device__ double block_min(double v, double* red)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -42,21 +45,23 @@ __device__ double block_min(double v, double* red)
     __syncthreads();
     if (lane == 0) red[wid] = v;
     __syncthreads();
-    double r = (lane < (kPrepThreads >> 5)) ? red[lane] : v;
+    double r = (lane < (TH >> 5)) ? red[lane] : v;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) r = fmin(r, __shfl_xor_sync(0xffffffffu, r, o));
     return r;
 }
 
 // <u v> over the series (u may alias v).
+template <int TH>
 __device__ double wdot(const double* __restrict__ w, const double* u, const double* v, int64_t N, double* red)
 {
     double acc = 0.0;
-    for (int64_t i = threadIdx.x; i < N; i += kPrepThreads) acc = fma(w[i] * u[i], v[i], acc);
-    return block_sum(acc, red);
+    for (int64_t i = threadIdx.x; i < N; i += TH) acc = fma(w[i] * u[i], v[i], acc);
+    return block_sum<TH>(acc, red);
 }
 
-__global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p)
+template <int TH>
+__global__ void __launch_bounds__(TH) prep_kernel(PrepParams p)
 {
     __shared__ double red[32];
     const int64_t b = blockIdx.x, N = p.N;
@@ -71,7 +76,7 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p)
 
     // ---- a1: validate, W = <1>, time origin --------------------------------------------
     double bad = 0.0, neg = 0.0, wsum = 0.0, tmin = INFINITY, tmax = -INFINITY;
-    for (int64_t i = threadIdx.x; i < N; i += kPrepThreads) {
+    for (int64_t i = threadIdx.x; i < N; i += TH) {
         double ti = t[i], xi = x[i], wi = w[i];
         if (!isfinite(ti) || !isfinite(xi) || !isfinite(wi)) bad = 1.0;
         if (wi < 0.0) neg = 1.0;
@@ -81,10 +86,10 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p)
         for (int j = 0; j < d; ++j)
             if (!isfinite(base[(int64_t)j * N + i])) bad = 1.0;
     }
-    bad = block_sum(bad + neg, red);
-    const double W = block_sum(wsum, red);
-    tmin = block_min(tmin, red);
-    tmax = -block_min(-tmax, red);
+    bad = block_sum<TH>(bad + neg, red);
+    const double W = block_sum<TH>(wsum, red);
+    tmin = block_min<TH>(tmin, red);
+    tmax = -block_min<TH>(-tmax, red);
     int status = 0;
     if (bad != 0.0 || !(W > 0.0) || !isfinite(W)) status = -2;  // FREDEC_EDATA
     const double t_mid = 0.5 * (tmin + tmax);
@@ -93,38 +98,38 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p)
     if (status == 0) {
         for (int j = 0; j < d; ++j) {
             double* v = psi + (int64_t)j * N;
-            for (int64_t i = threadIdx.x; i < N; i += kPrepThreads) v[i] = base[(int64_t)j * N + i];
+            for (int64_t i = threadIdx.x; i < N; i += TH) v[i] = base[(int64_t)j * N + i];
             __syncthreads();
-            const double n0 = wdot(w, v, v, N, red);
+            const double n0 = wdot<TH>(w, v, v, N, red);
             for (int sweep = 0; sweep < 2; ++sweep)
                 for (int k = 0; k < j; ++k) {
                     const double* q = psi + (int64_t)k * N;
-                    const double r = wdot(w, q, v, N, red);
-                    for (int64_t i = threadIdx.x; i < N; i += kPrepThreads) v[i] = fma(-r, q[i], v[i]);
+                    const double r = wdot<TH>(w, q, v, N, red);
+                    for (int64_t i = threadIdx.x; i < N; i += TH) v[i] = fma(-r, q[i], v[i]);
                     __syncthreads();
                 }
-            const double n1 = wdot(w, v, v, N, red);
+            const double n1 = wdot<TH>(w, v, v, N, red);
             if (!(n1 > kTauBase * n0)) {
                 status = -3;  // FREDEC_ESINGULAR (uniform across the block)
                 break;
             }
             const double inv = 1.0 / sqrt(n1);
-            for (int64_t i = threadIdx.x; i < N; i += kPrepThreads) v[i] *= inv;
+            for (int64_t i = threadIdx.x; i < N; i += TH) v[i] *= inv;
             __syncthreads();
         }
     }
     double chi2 = 0.0;
     if (status == 0) {
-        for (int64_t i = threadIdx.x; i < N; i += kPrepThreads) xt[i] = x[i];
+        for (int64_t i = threadIdx.x; i < N; i += TH) xt[i] = x[i];
         __syncthreads();
         for (int sweep = 0; sweep < 2; ++sweep)
             for (int k = 0; k < d; ++k) {
                 const double* q = psi + (int64_t)k * N;
-                const double r = wdot(w, q, xt, N, red);
-                for (int64_t i = threadIdx.x; i < N; i += kPrepThreads) xt[i] = fma(-r, q[i], xt[i]);
+                const double r = wdot<TH>(w, q, xt, N, red);
+                for (int64_t i = threadIdx.x; i < N; i += TH) xt[i] = fma(-r, q[i], xt[i]);
                 __syncthreads();
             }
-        chi2 = wdot(w, xt, xt, N, red);
+        chi2 = wdot<TH>(w, xt, xt, N, red);
     }
     if (threadIdx.x == 0) {
         info->W = W;
@@ -162,29 +167,34 @@ __global__ void __launch_bounds__(kTableThreads) table_kernel(TableParams p)
     double* grp = p.tab + ((b * p.n_pass + pass) * p.G4 + i / 4) * mma_group_doubles(H, p.NB);
     const int k = (int)(i & 3);
     const double* psi = p.psi + b * (int64_t)p.d * N;
-    for (int h = 1; h <= H; ++h) {
-        // alpha_h = 2 pi (h - 1/2) df t' in turns, range-reduced exactly
-        const double x = frac_prod((double)(2 * h - 1) * (0.5 * p.df), tc);
-        double c1, s1, c2, s2;
-        sincospi(2.0 * x, &s1, &c1);
-        sincospi(4.0 * x, &s2, &c2);
-        const int nt = (h - 1) >> 2, n0 = 2 * ((h - 1) & 3);
-        for (int f = 0; f < NF; ++f) {
-            double m, c = c1, s = s1;
-            if (f == 0) {
-                m = (pass == 0 && real) ? wi * p.xt[b * N + i] : 0.0;
-            } else if (f == NF - 1) {
-                m = pass == 0 ? 0.5 * wi : 0.0;
-                c = c2;
-                s = s2;
-            } else {
-                const int j = pass * p.NB + (f - 1);
-                m = (j < p.d && real) ? wi * psi[(int64_t)j * N + i] : 0.0;
+    // column tiles are stored in pairs (one 16-byte load per lane fetches the fragments of two): the
+    // thread writes the entries of tiles 2 tp and 2 tp + 1, i.e. of h and h + 4, as one double2
+    for (int tp = 0; tp < NT / 2; ++tp) {
+        for (int hh = 0; hh < 4; ++hh) {
+            double c1[2], s1[2], c2[2], s2[2];
+            for (int e = 0; e < 2; ++e) {
+                const int h = 8 * tp + 4 * e + hh + 1;
+                // alpha_h = 2 pi (h - 1/2) df t' in turns, range-reduced exactly
+                const double x = frac_prod((double)(2 * h - 1) * (0.5 * p.df), tc);
+                sincospi(2.0 * x, &s1[e], &c1[e]);
+                sincospi(4.0 * x, &s2[e], &c2[e]);
             }
-            // column tiles are stored in pairs (one 16-byte load per lane fetches the fragments of two)
-            double* tile = grp + (f * (NT / 2) + nt / 2) * 64 + (nt & 1);
-            tile[(n0 * 4 + k) * 2] = m * c;
-            tile[((n0 + 1) * 4 + k) * 2] = m * s;
+            const int n0 = 2 * hh;
+            for (int f = 0; f < NF; ++f) {
+                double m;
+                const bool dbl = f == NF - 1;  // the w family uses the doubled angles
+                if (f == 0) {
+                    m = (pass == 0 && real) ? wi * p.xt[b * N + i] : 0.0;
+                } else if (dbl) {
+                    m = pass == 0 ? 0.5 * wi : 0.0;
+                } else {
+                    const int j = pass * p.NB + (f - 1);
+                    m = (j < p.d && real) ? wi * psi[(int64_t)j * N + i] : 0.0;
+                }
+                double2* tile = reinterpret_cast<double2*>(grp + (f * (NT / 2) + tp) * 64);
+                tile[n0 * 4 + k] = make_double2(m * (dbl ? c2[0] : c1[0]), m * (dbl ? c2[1] : c1[1]));
+                tile[(n0 + 1) * 4 + k] = make_double2(m * (dbl ? s2[0] : s1[0]), m * (dbl ? s2[1] : s1[1]));
+            }
         }
     }
 }
@@ -200,7 +210,10 @@ cudaError_t launch_table(const TableParams& p, int64_t B, cudaStream_t stream)
 
 cudaError_t launch_prep(const PrepParams& p, int64_t B, cudaStream_t stream)
 {
-    prep_kernel<<<(unsigned)B, kPrepThreads, 0, stream>>>(p);
+    if (B >= 64 || p.N <= 2048)
+        prep_kernel<kPrepThreadsMin><<<(unsigned)B, kPrepThreadsMin, 0, stream>>>(p);
+    else
+        prep_kernel<kPrepThreadsMax><<<(unsigned)B, kPrepThreadsMax, 0, stream>>>(p);
     return cudaGetLastError();
 }
 
