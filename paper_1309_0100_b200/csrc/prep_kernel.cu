@@ -162,6 +162,7 @@ __global__ void __launch_bounds__(kTableThreads) table_kernel(TableParams p)
         r.t = tc;
         sincospi(2.0 * frac_prod(p.df * (double)(16 * H), tc), &r.su, &r.cu);  // one unit = 8 runs of 2H steps
         r.tcu = 2.0 * r.cu;
+        sincospi(2.0 * frac_prod(p.df * (double)(8 * H), tc), &r.s4, &r.c4);  // four runs
         p.srec[b * p.G4 * 4 + i] = r;
     }
     double* grp = p.tab + ((b * p.n_pass + pass) * p.G4 + i / 4) * mma_group_doubles(H, p.NB);

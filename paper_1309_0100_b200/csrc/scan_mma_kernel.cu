@@ -38,10 +38,11 @@
 //   seed warps (4, one per SM sub-partition)  wait until the MMA warps have left the slot
 //           (mbarrier "done"); one lane stages the table tile global -> shared by 1-D TMA
 //           (cp.async.bulk, mbarrier "tab"); then a5: seeds e^{i phi} for every (run of the
-//           round, observation of the tile) in A-fragment order -- one exact evaluation
-//           (range-reduced phase, table + short polynomial) at the round's first unit, one
-//           rotation to the second, then the two-term recurrence e_{u+1} = 2 cos(theta) e_u -
-//           e_{u-1} along the units -- and arrive on mbarrier "seed".
+//           round, observation of the tile) in A-fragment order -- per lane one exact evaluation
+//           (range-reduced phase, table + short polynomial) at the round's first unit for one run,
+//           a rotation by four runs for a second run, and for both one rotation to the second
+//           unit, then the two-term recurrence e_{u+1} = 2 cos(theta) e_u - e_{u-1} along the
+//           units -- and arrive on mbarrier "seed".
 //   MMA warps (8, two per sub-partition)  wait for "tab" and "seed"; per 4 observations:
 //           A fragments (seeds; double-angle seeds by 4 flops), B fragments (table),
 //           2 * NF * NT MMAs per unit; arrive on "done".  After the last tile of a round the
@@ -66,7 +67,7 @@ constexpr int kThreads = (kNW + kSeedWarps) * 32;
 // registers per thread after setmaxnreg: 128 * (2 * kRegsMma + kRegsSeed) <= 65536
 constexpr int kRegsMma = 208, kRegsSeed = 88;
 
-constexpr int kSeedGroups = 2;  // groups of 4 observations per seed warp and step at most (TI <= 32)
+constexpr int kSeedGroups = 2;  // groups of 4 observations per seed warp and step at most (TI <= 32): one per half warp
 
 // non-blocking: has the phase of the given parity completed?
 __device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity)
@@ -440,32 +441,23 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
         // ================= seed warps: table staging (a4) + seeds (a5) =====================
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsSeed));
         const int pw = wid - kNW;
-        const int m = lane >> 2, k = lane & 3;
+        // lane = (j, mp, k): group pw + 4 j of the slot, observation k of it, runs mp and mp + 4 of each
+        // unit.  One exact evaluation per lane and step serves two runs (the second by a rotation).
+        const int k = lane & 3, mp = (lane >> 2) & 3, ks = pw + kSeedWarps * (lane >> 4);
         const SeedRec* srec = p.srec + k;
         int slot = 0;
         uint32_t par = 0;  // parity of the slot's current use
         bool first_lap = true;
-        // this warp's records (groups pw, pw + 4 of the slot) are fetched one step ahead
-        double nt_[kSeedGroups], ncu[kSeedGroups], nsu[kSeedGroups], ntc[kSeedGroups];
+        // the lane's record is fetched one step ahead
+        SeedRec nxt = {0.0, 1.0, 0.0, 2.0, 1.0, 0.0};
         auto fetch = [&](const Cursor& cc) {
             const int ng = (int)min((int64_t)KS, p.G4 - (int64_t)cc.tile * KS);
-            const SeedRec* rp = srec + (cc.b * p.G4 + (int64_t)cc.tile * KS + pw) * 4;
-#pragma unroll
-            for (int j = 0; j < kSeedGroups; ++j) {
-                if (pw + kSeedWarps * j < ng) {
-                    const SeedRec* r = rp + kSeedWarps * j * 4;
-                    nt_[j] = r->t; ncu[j] = r->cu; nsu[j] = r->su; ntc[j] = r->tcu;
-                }
-            }
+            if (ks < ng) nxt = srec[(cc.b * p.G4 + (int64_t)cc.tile * KS + ks) * 4];
         };
         if (c.valid) fetch(c);
         while (c.valid) {
             const int ngrp = (int)min((int64_t)KS, p.G4 - (int64_t)c.tile * KS);
-            double rt[kSeedGroups], rcu[kSeedGroups], rsu[kSeedGroups], rtc[kSeedGroups];
-#pragma unroll
-            for (int j = 0; j < kSeedGroups; ++j) {
-                rt[j] = nt_[j]; rcu[j] = ncu[j]; rsu[j] = nsu[j]; rtc[j] = ntc[j];
-            }
+            const SeedRec r = nxt;
             const int nunits = c.n;
             const int64_t u0 = c.u;
             const double* tab_src = p.tab + ((c.b * p.n_pass + p.pass) * p.G4 + (int64_t)c.tile * KS) * GROUP;
@@ -478,33 +470,34 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
                 mbar_expect_tx(&bar_tab[slot], bytes);
                 bulk_g2s(base, tab_src, bytes, &bar_tab[slot]);
             }
-            // centre of run m of the round's first unit: f_c = f0 + (run R + H - 1/2) df   (S1)
-            const double kc = (double)((u0 * 8 + m) * R + H) - 0.5;
-            const double fc = fma(kc, p.df, p.f0);
-            double2* sb = reinterpret_cast<double2*>(base + tab_bytes) + lane;
+            if (ks < ngrp) {
+                // centre of run mp of the round's first unit: f_c = f0 + (run R + H - 1/2) df   (S1)
+                const double kc = (double)((u0 * 8 + mp) * R + H) - 0.5;
+                const double fc = fma(kc, p.df, p.f0);
+                // unit 0 of run mp exactly; run mp + 4 by one rotation; per run: unit 1 by one rotation,
+                // then the two-term recurrence e_{u+1} = 2 cos(theta) e_u - e_{u-1} (theta = one unit step)
+                double ca0, sa0;
+                sincos_turns(frac_prod(fc, r.t), trig64, ca0, sa0);
+                double cb0 = ca0, sb0 = sa0;
+                rotate(cb0, sb0, r.c4, r.s4);
+                double ca1 = ca0, sa1 = sa0, cb1 = cb0, sb1 = sb0;
+                rotate(ca1, sa1, r.cu, r.su);
+                rotate(cb1, sb1, r.cu, r.su);
+                double2* da = reinterpret_cast<double2*>(base + tab_bytes) + (size_t)ks * CAP * 32 + mp * 4 + k;
+                double2* db = da + 16;  // run mp + 4
+                da[0] = make_double2(ca0, sa0);
+                db[0] = make_double2(cb0, sb0);
+                da[32] = make_double2(ca1, sa1);
+                db[32] = make_double2(cb1, sb1);
 #pragma unroll
-            for (int j = 0; j < kSeedGroups; ++j) {
-                const int ks = pw + kSeedWarps * j;
-                if (ks < ngrp) {
-                    // unit 0 exactly, unit 1 by one rotation, then the two-term recurrence
-                    // e_{u+1} = 2 cos(theta) e_u - e_{u-1} along the units (theta = one unit step)
-                    double c0, s0;
-                    sincos_turns(frac_prod(fc, rt[j]), trig64, c0, s0);
-                    double c1 = c0, s1 = s0;
-                    rotate(c1, s1, rcu[j], rsu[j]);
-                    double2* dst = sb + (size_t)ks * CAP * 32;
-                    dst[0] = make_double2(c0, s0);
-                    dst[32] = make_double2(c1, s1);
-#pragma unroll
-                    for (int u = 2; u < CAP; ++u) {
-                        if (u >= nunits) break;  // rounds of fewer units need fewer seeds
-                        const double c2 = fma(rtc[j], c1, -c0), s2 = fma(rtc[j], s1, -s0);
-                        dst[u * 32] = make_double2(c2, s2);
-                        c0 = c1;
-                        s0 = s1;
-                        c1 = c2;
-                        s1 = s2;
-                    }
+                for (int u = 2; u < CAP; ++u) {
+                    if (u >= nunits) break;  // rounds of fewer units need fewer seeds
+                    const double ca2 = fma(r.tcu, ca1, -ca0), sa2 = fma(r.tcu, sa1, -sa0);
+                    const double cb2 = fma(r.tcu, cb1, -cb0), sb2 = fma(r.tcu, sb1, -sb0);
+                    da[u * 32] = make_double2(ca2, sa2);
+                    db[u * 32] = make_double2(cb2, sb2);
+                    ca0 = ca1; sa0 = sa1; ca1 = ca2; sa1 = sa2;
+                    cb0 = cb1; sb0 = sb1; cb1 = cb2; sb1 = sb2;
                 }
             }
             __syncwarp();

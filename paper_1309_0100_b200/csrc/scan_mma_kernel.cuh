@@ -23,9 +23,10 @@ __host__ __device__ constexpr int mma_nf(int NB) { return NB + 2; }
 __host__ __device__ constexpr int mma_group_doubles(int H, int NB) { return mma_nf(NB) * mma_nt(H) * 32; }
 
 // Per-observation seed record: t', (cos, sin) of the rotation by one unit (8 runs = 8R grid
-// steps), and 2 cos of it (coefficient of the two-term recurrence along the units).
-struct __align__(32) SeedRec {
-    double t, cu, su, tcu;
+// steps), 2 cos of it (coefficient of the two-term recurrence along the units), and (cos, sin)
+// of the rotation by four runs (4R grid steps).
+struct __align__(16) SeedRec {
+    double t, cu, su, tcu, c4, s4;
 };
 
 struct MmaScanParams {
