@@ -65,7 +65,7 @@ constexpr int kNW = 8;         // MMA warps per CTA (two per SM sub-partition)
 constexpr int kSeedWarps = 4;  // seed warps per CTA (one per SM sub-partition)
 constexpr int kThreads = (kNW + kSeedWarps) * 32;
 // registers per thread after setmaxnreg: 128 * (2 * kRegsMma + kRegsSeed) <= 65536
-constexpr int kRegsMma = 208, kRegsSeed = 88;
+constexpr int kRegsMma = 216, kRegsSeed = 72;
 
 constexpr int kSeedGroups = 2;  // groups of 4 observations per seed warp and step at most (TI <= 32): one per half warp
 
