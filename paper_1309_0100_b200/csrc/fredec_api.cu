@@ -80,7 +80,7 @@ struct State {
     cudaStream_t stream = nullptr;
     cudaEvent_t ev[kNumEvents] = {};
     DevBuf in_t, in_x, in_w, in_base, in_z, out_z, out_idx, out_chi2;
-    DevBuf gram, rf, p1_base, p1_freq, p1_z, p1_idx, p1_stats, tab, srec, psi, xt, info, ws, red, part_z, part_i, count, sink;
+    DevBuf gram, rf, part, p1_base, p1_freq, p1_z, p1_idx, p1_stats, tab, srec, psi, xt, info, ws, red, part_z, part_i, count, sink;
     HostBuf h_info, h_count;
     int last_cuda = 0;
     double timing[4] = {0, 0, 0, 0};
@@ -273,10 +273,23 @@ int enqueue_series_mma(Call& c, const double* dt, const double* dx, const double
     }
     CK(g.red.reserve((size_t)sp.grid * cfg.NW * mma_red_doubles(NB) * 8));
     sp.red = g.red.as<double>();
+    // one series in one pass: full rounds per CTA + left-over rounds cut across the observations
+    sp.shared = (B == 1 && n_pass == 1 && U >= (int64_t)cfg.NW * cfg.NOCT * g.sm_count) ? 1 : 0;  // >= 1 full round per CTA
+    sp.F = 0;
+    sp.Rt = 0;
+    sp.part = nullptr;
+    if (sp.shared) {
+        const int64_t cap = (int64_t)cfg.NW * cfg.NOCT;
+        sp.grid = g.sm_count;
+        sp.F = (int)(U / (cap * sp.grid));
+        sp.Rt = (int)((U - (int64_t)sp.F * cap * sp.grid + cap - 1) / cap);
+        CK(g.part.reserve((size_t)2 * sp.grid * cfg.NW * mma_part_doubles(NB) * 8));
+        sp.part = g.part.as<double>();
+    }
     for (int pass = 0; pass < n_pass; ++pass) {
         sp.pass = pass;
         CK(launch_mma_scan(NB, sp, st));
-        g.launches += 1;
+        g.launches += (sp.shared && sp.Rt > 0) ? 2 : 1;  // + the tail-solve kernel
     }
     CK(cudaEventRecord(g.ev[3], st));
     c.B = B;
@@ -812,7 +825,7 @@ int fredec_fp64_peak(int64_t iters, double* tflops_out, double* ms_out)
 
 int fredec_shutdown(void)
 {
-    DevBuf* bufs[] = {&g.in_t, &g.in_x, &g.in_w, &g.in_base, &g.in_z, &g.out_z, &g.out_idx, &g.out_chi2, &g.gram, &g.rf, &g.p1_base, &g.p1_freq, &g.p1_z, &g.p1_idx, &g.p1_stats, &g.tab, &g.srec,
+    DevBuf* bufs[] = {&g.in_t, &g.in_x, &g.in_w, &g.in_base, &g.in_z, &g.out_z, &g.out_idx, &g.out_chi2, &g.gram, &g.rf, &g.part, &g.p1_base, &g.p1_freq, &g.p1_z, &g.p1_idx, &g.p1_stats, &g.tab, &g.srec,
                       &g.psi,  &g.xt,   &g.info, &g.ws, &g.red,     &g.part_z, &g.part_i, &g.count, &g.sink};
     for (DevBuf* b : bufs) b->release();
     g.h_info.release();

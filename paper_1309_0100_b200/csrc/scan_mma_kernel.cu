@@ -51,6 +51,10 @@
 // Rounds hold a power of two of units.  A round of fewer units than MMA warps (the tail of a
 // CTA's range, or a short grid) splits the observations between the warps that share a unit
 // (a8); their partial sums are added in fixed order through a per-CTA scratch in global memory.
+// For one long series (at least one full round per CTA) the left-over rounds are instead cut
+// across the observations BETWEEN CTAs ("shared" mode of the Cursor): every CTA ends with a piece
+// of a left-over round, writes its partial sums to a workspace, and tail_solve_kernel adds the
+// pieces in fixed order and solves -- also row a8, at the scale of the chip.
 //
 // The seed warps run up to NS steps ahead of the MMA warps, so the latency of the seed chains
 // (which share the FP64 pipe with the MMAs) is off the MMA warps' critical path.
@@ -95,17 +99,51 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar)
         : "d"(a), "d"(b))
 
 // Position of a CTA in its sequence of (round, tile) steps.  The seed warps and the MMA warps
-// walk the same sequence, each with its own cursor.
+// walk the same sequence, each with its own cursor.  Two ways of cutting the work:
+//   ranges  (several series, or several passes): the CTA owns a contiguous range of units and
+//           cuts it into rounds of a power of two of units; every round covers all tiles.
+//   shared  (one series, one pass): every CTA first runs F full rounds of `cap` units of its own;
+//           the rounds that are left over (fewer than one per CTA) are cut ACROSS THE OBSERVATIONS:
+//           the CTA takes a contiguous piece of the sequence (left-over round, tile), i.e. at most
+//           two SEGMENTS (round, tile range), whose partial sums go to a workspace (seg >= 0) and
+//           are added and solved by tail_solve_kernel.  All CTAs then finish together, and no round
+//           streams the table for a fraction of the work.
 struct Cursor {
-    int64_t g, g_end;  // next unit after this round / end of the CTA's range (global numbering)
+    int64_t g, g_end;  // ranges: first unit of this round / end of the CTA's range (global numbering)
     int64_t b, u;      // series and first unit (within the series) of the current round
     int n;             // units in the current round
-    int tile;          // tile within the round
-    int step;          // steps taken so far: selects the stage and the seed buffer
+    int tile;          // current tile
+    int tile_end;      // end of the round's tile range
+    int seg;           // >= 0: a segment of a left-over round (partial sums), -1: a whole round
     bool valid;
+    // shared mode
+    bool shared;
+    int it, F, ntiles_, cap_;
+    int64_t s0, s1, tail_u0;
 
     __device__ __forceinline__ void set_round(int64_t U, int cap)
     {
+        if (shared) {
+            n = cap_;
+            b = 0;
+            if (it < F) {
+                u = ((int64_t)blockIdx.x * F + it) * cap_;
+                tile = 0;
+                tile_end = ntiles_;
+                seg = -1;
+                valid = true;
+            } else {
+                const int j = it - F;
+                const int64_t r = s0 / ntiles_ + j;
+                const int64_t lo = max(s0, r * ntiles_), hi = min(s1, (r + 1) * ntiles_);
+                valid = j < 2 && lo < hi;
+                u = tail_u0 + r * cap_;
+                tile = (int)(lo - r * ntiles_);
+                tile_end = (int)(hi - r * ntiles_);
+                seg = 2 * (int)blockIdx.x + j;
+            }
+            return;
+        }
         b = g / U;
         u = g - b * U;
         int64_t m = U - u;
@@ -113,31 +151,50 @@ struct Cursor {
         n = m < cap ? (int)m : cap;
         n = 1 << (31 - __clz(n));  // a power of two: rounds smaller than kNW split the observations
     }
-    __device__ __forceinline__ void init(int64_t g0, int64_t g1, int64_t U, int cap)
+    __device__ __forceinline__ void init(const MmaScanParams& p, int ntiles, int cap)
     {
-        g = g0;
-        g_end = g1;
+        shared = p.shared != 0;
         tile = 0;
-        step = 0;
-        valid = g < g_end;
+        tile_end = ntiles;
+        seg = -1;
         b = u = 0;
         n = 0;
-        if (valid) set_round(U, cap);
+        g = g_end = 0;
+        it = 0;
+        F = p.F;
+        ntiles_ = ntiles;
+        cap_ = cap;
+        s0 = s1 = tail_u0 = 0;
+        if (shared) {
+            const int64_t S = (int64_t)p.Rt * ntiles;
+            s0 = (int64_t)blockIdx.x * S / p.grid;
+            s1 = (int64_t)(blockIdx.x + 1) * S / p.grid;
+            tail_u0 = (int64_t)p.grid * F * cap;
+            set_round(p.U, cap);
+            return;
+        }
+        g = (int64_t)blockIdx.x * p.T / p.grid;
+        g_end = (int64_t)(blockIdx.x + 1) * p.T / p.grid;
+        valid = g < g_end;
+        if (valid) set_round(p.U, cap);
     }
     __device__ __forceinline__ void next_round(int64_t U, int cap)
     {
+        if (shared) {
+            ++it;
+            set_round(U, cap);
+            return;
+        }
         g += n;
         valid = g < g_end;
         if (valid) set_round(U, cap);
     }
     __device__ __forceinline__ void advance(int ntiles, int64_t U, int cap)
     {
-        ++step;
-        if (++tile == ntiles) {
+        if (++tile == tile_end) {
             tile = 0;
-            g += n;
-            valid = g < g_end;
-            if (valid) set_round(U, cap);
+            tile_end = ntiles;
+            next_round(U, cap);
         }
     }
 };
@@ -235,13 +292,14 @@ __device__ __forceinline__ void mma_group(Tiles<H, NOCT, NB>& acc, const double2
 template <int CNT, int H, int NOCT, int NB>
 __device__ __forceinline__ void round_mma(Tiles<H, NOCT, NB>& acc, RingPos& rp, const unsigned char* smem,
                                           size_t slot_bytes, size_t tab_bytes, int NS, int KS, int64_t G4,
-                                          WarpRole role, int lane, uint64_t* bar_tab, uint64_t* bar_seed,
-                                          uint64_t* bar_done)
+                                          int tile0, int tile1, WarpRole role, int lane, uint64_t* bar_tab,
+                                          uint64_t* bar_seed, uint64_t* bar_done)
 {
     constexpr int NT = H / 4, NF = NB + 2, GROUP2 = NF * NT * 16, CAP = kNW * NOCT;  // GROUP2: double2 per group
+    const int64_t g_end = min((int64_t)tile1 * KS, G4);
 #pragma unroll 1
-    for (int64_t g = 0; g < G4; g += KS) {
-        const int ngrp = (int)min((int64_t)KS, G4 - g);
+    for (int64_t g = (int64_t)tile0 * KS; g < g_end; g += KS) {
+        const int ngrp = (int)min((int64_t)KS, g_end - g);
         if (!rp.ready) {
             mbar_wait(&bar_tab[rp.slot], rp.par);
             mbar_wait(&bar_seed[rp.slot], rp.par);
@@ -433,9 +491,8 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
     }
     __syncthreads();
 
-    const int64_t g0 = (int64_t)blockIdx.x * p.T / p.grid, g1 = (int64_t)(blockIdx.x + 1) * p.T / p.grid;
     Cursor c;
-    c.init(g0, g1, U, CAP);
+    c.init(p, ntiles, CAP);
 
     if (wid >= kNW) {
         // ================= seed warps: table staging (a4) + seeds (a5) =====================
@@ -517,7 +574,8 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
         while (c.valid) {  // one round per iteration
             const WarpRole role = warp_role(c.n, wid);
 #define FREDEC_ROUND(CNT) \
-    round_mma<CNT>(acc, rp, smem_raw, slot_bytes, tab_bytes, NS, KS, p.G4, role, lane, bar_tab, bar_seed, bar_done)
+    round_mma<CNT>(acc, rp, smem_raw, slot_bytes, tab_bytes, NS, KS, p.G4, c.tile, c.tile_end, role, lane, bar_tab, \
+                   bar_seed, bar_done)
             if (NOCT == 1 || role.cnt == 1) {
                 FREDEC_ROUND(1);
             } else if (NOCT == 2 || role.cnt == 2) {
@@ -560,11 +618,62 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
                     }
                 }
             }
-            if (solve) solve_and_store<H, NOCT, NB>(acc, p, c.b, c.u + role.off, role.cnt, lane);
+            if (c.seg >= 0) {
+                // a segment of a left-over round: the sums over its tiles go to the workspace
+                constexpr int ACCW = NOCT * 2 * NF * NT * 2;
+                double* dst = p.part + ((size_t)c.seg * kNW + wid) * (ACCW * 32) + lane;
+#pragma unroll
+                for (int o = 0; o < NOCT; ++o)
+#pragma unroll
+                    for (int x = 0; x < 2; ++x)
+#pragma unroll
+                        for (int f = 0; f < NF; ++f)
+#pragma unroll
+                            for (int t = 0; t < NT; ++t) {
+                                __stcg(dst + ((((o * 2 + x) * NF + f) * NT + t) * 2 + 0) * 32, acc.v[o][x][f][t][0]);
+                                __stcg(dst + ((((o * 2 + x) * NF + f) * NT + t) * 2 + 1) * 32, acc.v[o][x][f][t][1]);
+                            }
+            } else if (solve) {
+                solve_and_store<H, NOCT, NB>(acc, p, c.b, c.u + role.off, role.cnt, lane);
+            }
             acc.clear();
             c.next_round(U, CAP);
         }
     }
+}
+
+// Shared mode: adds the partial sums of the segments of left-over round blockIdx.x in the order of
+// the CTAs that produced them (fixed: bitwise reproducible), then a9/a10 as in the scan kernel.
+template <int H, int NOCT, int NB>
+__global__ void __launch_bounds__(kNW * 32) tail_solve_kernel(MmaScanParams p)
+{
+    constexpr int NT = H / 4, NF = NB + 2, CAP = kNW * NOCT, ACCW = NOCT * 2 * NF * NT * 2;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int KS = p.TI / 4;
+    const int ntiles = (int)((p.G4 + KS - 1) / KS);
+    const int64_t r = blockIdx.x, S = (int64_t)p.Rt * ntiles;
+    Tiles<H, NOCT, NB> acc;
+    acc.clear();
+    for (int cta = 0; cta < p.grid; ++cta) {
+        const int64_t s0 = (int64_t)cta * S / p.grid, s1 = (int64_t)(cta + 1) * S / p.grid;
+        const int64_t j = r - s0 / ntiles;
+        if (j < 0 || j > 1) continue;
+        if (max(s0, r * ntiles) >= min(s1, (r + 1) * ntiles)) continue;
+        const double* src = p.part + ((size_t)(2 * cta + (int)j) * kNW + wid) * (ACCW * 32) + lane;
+#pragma unroll
+        for (int o = 0; o < NOCT; ++o)
+#pragma unroll
+            for (int x = 0; x < 2; ++x)
+#pragma unroll
+                for (int f = 0; f < NF; ++f)
+#pragma unroll
+                    for (int t = 0; t < NT; ++t) {
+                        acc.v[o][x][f][t][0] += __ldcg(src + ((((o * 2 + x) * NF + f) * NT + t) * 2 + 0) * 32);
+                        acc.v[o][x][f][t][1] += __ldcg(src + ((((o * 2 + x) * NF + f) * NT + t) * 2 + 1) * 32);
+                    }
+    }
+    const int64_t u = (int64_t)p.grid * p.F * CAP + r * CAP + wid * NOCT;
+    solve_and_store<H, NOCT, NB>(acc, p, 0, u, NOCT, lane);
 }
 
 template <int H, int NOCT, int NB>
@@ -580,6 +689,9 @@ cudaError_t launch_one(const MmaScanParams& p, cudaStream_t stream)
     }
     if (p.NS < 2 || p.NS > kMmaMaxSlots || p.TI < 4 || p.TI % 4 || p.TI > 16 * kSeedGroups) return cudaErrorInvalidValue;
     scan_mma_kernel<H, NOCT, NB><<<p.grid, kThreads, smem, stream>>>(p);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess || !p.shared || p.Rt == 0) return e;
+    tail_solve_kernel<H, NOCT, NB><<<p.Rt, kNW * 32, 0, stream>>>(p);
     return cudaGetLastError();
 }
 
@@ -608,6 +720,12 @@ size_t mma_red_doubles(int NB)
 {
     const MmaScanConfig c = mma_scan_config(NB);
     return (size_t)2 * mma_nf(NB) * mma_nt(c.H) * 2 * 32;
+}
+
+size_t mma_part_doubles(int NB)
+{
+    const MmaScanConfig c = mma_scan_config(NB);
+    return (size_t)c.NOCT * 2 * mma_nf(NB) * mma_nt(c.H) * 2 * 32;
 }
 
 cudaError_t launch_mma_scan(int NB, const MmaScanParams& p, cudaStream_t stream)

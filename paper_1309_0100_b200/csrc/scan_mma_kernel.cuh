@@ -36,6 +36,7 @@ struct MmaScanParams {
     double* z;               // [B][K] out
     double* ws;              // [B][7][Kpad] partial sums between passes (nullptr if n_pass == 1)
     double* red;             // [grid][MMA warps][mma_red_doubles] scratch of the observation-split reduction
+    double* part;            // shared mode: [2 grid][MMA warps][mma_part_doubles] partial sums of the segments
     int64_t N, K, Kpad;
     int64_t G4;  // groups of 4 observations per series = ceil(N / 4)
     int64_t U;   // units per series = ceil(K / (8 R))
@@ -45,6 +46,9 @@ struct MmaScanParams {
     int TI;    // observations per shared-memory slot (multiple of 4)
     int NS;    // slots of the (table tile, seeds) ring in shared memory
     int grid;  // CTAs (persistent; each owns a contiguous range of units)
+    // shared mode (one series, one pass; see Cursor in scan_mma_kernel.cu): F full rounds per CTA, then
+    // Rt left-over rounds cut across the observations and finished by the tail-solve kernel
+    int shared, F, Rt;
 };
 
 struct MmaScanConfig {
@@ -55,7 +59,8 @@ struct MmaScanConfig {
 constexpr int kMmaMaxNB = 9;
 MmaScanConfig mma_scan_config(int NB);
 size_t mma_scan_slot_bytes(int NB, int TI);
-size_t mma_red_doubles(int NB);  // per MMA warp: the accumulators of one unit  // one ring slot; the kernel needs NS of them
+size_t mma_red_doubles(int NB);  // per MMA warp: the accumulators of one unit
+size_t mma_part_doubles(int NB); // per MMA warp: all its accumulators  // one ring slot; the kernel needs NS of them
 constexpr int kMmaMaxSlots = 8;
 cudaError_t launch_mma_scan(int NB, const MmaScanParams& p, cudaStream_t stream);
 

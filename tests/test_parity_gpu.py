@@ -339,3 +339,23 @@ def test_long_series_many_ring_laps(fr, oracle_mod):
     z = gpu_scan(fr, t, x, w, base, f0, df, K)
     assert_parity(z, z_ref, "long series")
     assert abs((f0 + df * int(np.argmax(z))) - 0.0371) < 2 * df
+
+
+@pytest.mark.parametrize("d,N", [(2, 150), (0, 90), (3, 131), (9, 70), (1, 33)])
+def test_shared_tail_mode(fr, oracle_mod, d, N):
+    """One series with at least one full round per SM: every CTA runs its full rounds, the left-over
+    rounds are cut across the observations into segments whose partial sums the tail-solve kernel
+    adds.  Grid sizes chosen for 148 SMs: one full round per CTA, then left-over rounds the last of
+    which is only partly filled; few tiles per round, so that segments start and end inside rounds."""
+    import torch
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    run = 32 if d <= 2 else 16                       # frequencies per run (DESIGN.md section 5)
+    cap = 16 if d in (0, 3) else 8                   # units per round
+    units = sms * cap + 5 * cap + 3
+    K = units * 8 * run - 7
+    t, x, w, base = inputs.random_series(7000 + d, N, d, t_span=60.0)
+    f0, df = 0.2, 3.0 / K                            # clear of f -> 0 and of the base frequencies (S6)
+    z_ref = oracle_mod.scan(t, x, w, base, f0, df, K, threads=0)
+    z = gpu_scan(fr, t, x, w, base, f0, df, K)
+    assert_parity(z, z_ref, f"shared mode d={d}")
+    assert np.array_equal(z, gpu_scan(fr, t, x, w, base, f0, df, K))      # fixed summation order
