@@ -654,7 +654,10 @@ __global__ void __launch_bounds__(kNW * 32) tail_solve_kernel(MmaScanParams p)
     const int64_t r = blockIdx.x, S = (int64_t)p.Rt * ntiles;
     Tiles<H, NOCT, NB> acc;
     acc.clear();
-    for (int cta = 0; cta < p.grid; ++cta) {
+    // only the CTAs whose piece [cta S / grid, (cta + 1) S / grid) can meet the round's steps [r, r + 1) ntiles
+    const int c_lo = (int)max((int64_t)0, r * ntiles * p.grid / S - 1);
+    const int c_hi = (int)min((int64_t)p.grid - 1, ((r + 1) * ntiles * p.grid + S - 1) / S);
+    for (int cta = c_lo; cta <= c_hi; ++cta) {
         const int64_t s0 = (int64_t)cta * S / p.grid, s1 = (int64_t)(cta + 1) * S / p.grid;
         const int64_t j = r - s0 / ntiles;
         if (j < 0 || j > 1) continue;
