@@ -232,20 +232,6 @@ int FN(oracle_scan)(const double *t, const double *x, const double *w, int64_t N
     return status;
 }
 
-int FN(oracle_scan_batched)(const double *t, const double *x, const double *w, int64_t B, int64_t N,
-                            const double *base_funcs, int32_t d, double f0, double df, int64_t K,
-                            double *z_out)
-{
-    if (B < 1) return ORACLE_EINVAL;
-    for (int64_t b = 0; b < B; ++b) {
-        int rc = FN(oracle_scan)(t + b * N, x + b * N, w + b * N, N,
-                                 d > 0 ? base_funcs + b * (int64_t)d * N : NULL, d, f0, df, K,
-                                 z_out + b * K);
-        if (rc) return rc;
-    }
-    return ORACLE_OK;
-}
-
 /* Trigonometric averages of PAPER.md:242-262 (section 5) at an arbitrary list of M frequencies
  * (omega_j = 2 pi f_j), per pair with libm on the exactly reduced phase, summed in index order.
  * out [M][10], in the paper's order: system (19)
@@ -311,16 +297,6 @@ int oracle_topk(const double *z, int64_t K, int32_t k, int64_t *idx_out)
     for (int j = 0; j < k; ++j) idx_out[j] = j < found ? peaks[j].idx : -1;
     free(peaks);
     return found;
-}
-
-int oracle_topk_batched(const double *z, int64_t B, int64_t K, int32_t k, int64_t *idx_out)
-{
-    if (B < 1) return ORACLE_EINVAL;
-    for (int64_t b = 0; b < B; ++b) {
-        int rc = oracle_topk(z + b * K, K, k, idx_out + b * k);
-        if (rc < 0) return rc;
-    }
-    return ORACLE_OK;
 }
 
 int oracle_num_threads(void)

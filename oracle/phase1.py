@@ -2,7 +2,8 @@
 oracle's scan / topk).  TEST INFRASTRUCTURE ONLY (see oracle/__init__.py); shares no code with the
 CUDA path.  Each function follows the passage it cites, in the paper's order and notation.
 
-Pins (tests/test_oracle_pins.py): zstat against (N_H/2) ln(l_base/l_alt) with both l from QR fits;
+Pins (tests/test_phase1_pins.py; subset_fits: tests/test_subset_pins.py; refine:
+tests/test_refine_pins.py): zstat against (N_H/2) ln(l_base/l_alt) with both l from QR fits;
 T_eff against the closed form for evenly spaced, equally weighted times; fap1 against hand values;
 phase 1 on constructed series whose outcome the rules fix.  The coefficient A~_1 of eq. 13 and the
 readings P1-P4 are not fixed by the paper: parity unpinned for those.

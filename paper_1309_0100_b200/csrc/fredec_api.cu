@@ -81,12 +81,22 @@ struct State {
     cudaEvent_t ev[kNumEvents] = {};
     DevBuf in_t, in_x, in_w, in_base, in_z, out_z, out_idx, out_chi2;
     DevBuf gram, rf, part, p1_base, p1_freq, p1_z, p1_idx, p1_stats, tab, srec, psi, xt, info, ws, red, part_z, part_i, count, sink;
-    HostBuf h_info, h_count;
+    HostBuf h_info, h_count, h_flag;
+    DevBuf flag;
     int last_cuda = 0;
     double timing[4] = {0, 0, 0, 0};
     int launches = 0;
 };
 State g;
+
+// Error path of every entry point: copies or kernels that touch the caller's buffers may still be
+// queued on the stream; wait for them so that "the library keeps no pointer after return" also holds
+// when a call fails (the result of the wait itself is ignored).
+void drain_stream()
+{
+    if (g.ready) (void)cudaStreamSynchronize(g.stream);
+    (void)cudaGetLastError();
+}
 
 #define CK(expr)                                \
     do {                                        \
@@ -94,6 +104,7 @@ State g;
         if (e__ != cudaSuccess) {               \
             g.last_cuda = (int)e__;             \
             (void)cudaGetLastError();           \
+            drain_stream();                     \
             return FREDEC_ECUDA;                \
         }                                       \
     } while (0)
@@ -492,6 +503,18 @@ int device_bandwidth(const double* dt, const double* dw, int64_t N, double out4[
     return out4[3] != 0.0 ? FREDEC_EDATA : FREDEC_OK;
 }
 
+// enqueues the "all finite" check of a device array; the flag is read by flag_status() after the
+// call's final synchronisation
+int enqueue_finite_check(const double* dv, int64_t n)
+{
+    CK(g.flag.reserve(sizeof(int)));
+    CK(g.h_flag.reserve(sizeof(int)));
+    CK(launch_finite_flag(dv, n, g.flag.as<int>(), g.stream));
+    CK(cudaMemcpyAsync(g.h_flag.p, g.flag.p, sizeof(int), cudaMemcpyDeviceToHost, g.stream));
+    return FREDEC_OK;
+}
+int flag_status() { return *static_cast<const int*>(g.h_flag.p) != 0 ? FREDEC_EDATA : FREDEC_OK; }
+
 struct PoolEntry {
     int64_t idx;
     double z, fap;
@@ -682,13 +705,14 @@ int fredec_trig_averages(const double* t, const double* x, const double* w, int6
     if ((rc = stage_in(freqs, (size_t)M, g.in_z, &dfr))) return rc;
     double *dout, *hout;
     if ((rc = stage_out(out, (size_t)M * kTrigCols, g.out_z, &dout, &hout))) return rc;
+    if ((rc = enqueue_finite_check(dfr, M))) return rc;
     CK(launch_trig_averages(dt, dx, dw, N, dfr, M, dout, g.stream));
-    g.launches += 1;
+    g.launches += 2;
     if (hout) CK(cudaMemcpyAsync(hout, dout, (size_t)M * kTrigCols * 8, cudaMemcpyDeviceToHost, g.stream));
     CK(cudaEventRecord(g.ev[6], g.stream));
     CK(cudaStreamSynchronize(g.stream));
     g.timing[3] = ev_ms(0, 6);
-    return FREDEC_OK;
+    return flag_status();
 }
 
 int fredec_subset_fits(const double* t, const double* x, const double* w, int64_t N, const double* freqs, int32_t n,
@@ -709,18 +733,19 @@ int fredec_subset_fits(const double* t, const double* x, const double* w, int64_
     if ((rc = stage_out(l_out, total, g.out_z, &dl, &hl))) return rc;
     CK(g.p1_base.reserve((size_t)M * N * 8));
     CK(g.gram.reserve((size_t)(M + 1) * (M + 1) * 8));
+    if ((rc = enqueue_finite_check(dfr, n))) return rc;
     CK(launch_sin_base(dt, N, dfr, n, g.p1_base.as<double>(), st));
     CK(launch_gram(g.p1_base.as<double>(), dx, dw, N, M, g.gram.as<double>(), st));
     CK(cudaEventRecord(g.ev[2], st));
     CK(launch_subset_fits(g.gram.as<double>(), n, dl, g.sm_count, st));
     CK(cudaEventRecord(g.ev[3], st));
-    g.launches += 3;
+    g.launches += 4;
     if (hl) CK(cudaMemcpyAsync(hl, dl, total * 8, cudaMemcpyDeviceToHost, st));
     CK(cudaEventRecord(g.ev[6], st));
     CK(cudaStreamSynchronize(st));
     g.timing[1] = ev_ms(2, 3);
     g.timing[3] = ev_ms(0, 6);
-    return FREDEC_OK;
+    return flag_status();
 }
 
 int fredec_refine(const double* t, const double* x, const double* w, int64_t N, double* freqs, int32_t n,
@@ -751,6 +776,9 @@ int fredec_refine(const double* t, const double* x, const double* w, int64_t N, 
     double* out2 = dstep + n;            // [2] linear fit, [2] Gauss-Newton step
     const bool freqs_dev = on_device(freqs);
     CK(cudaMemcpyAsync(dfreq, freqs, (size_t)n * 8, freqs_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+    if ((rc = enqueue_finite_check(dfreq, n))) return rc;
+    CK(cudaStreamSynchronize(st));
+    if ((rc = flag_status())) return rc;
     std::vector<double> hstep((size_t)n);
     double hout[4];
     int iters = 0, launches = 1;
@@ -829,6 +857,8 @@ int fredec_shutdown(void)
                       &g.psi,  &g.xt,   &g.info, &g.ws, &g.red,     &g.part_z, &g.part_i, &g.count, &g.sink};
     for (DevBuf* b : bufs) b->release();
     g.h_info.release();
+    g.h_flag.release();
+    g.flag.release();
     g.h_count.release();
     if (g.ready)
         for (int i = 0; i < kNumEvents; ++i) cudaEventDestroy(g.ev[i]);

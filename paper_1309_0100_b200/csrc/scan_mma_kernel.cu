@@ -602,7 +602,11 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
                             }
                     solve = false;
                 }
-                asm volatile("bar.sync %0, %1;" ::"r"(1 + role.off), "r"(role.S * 32) : "memory");
+                // Named barrier of the S warps that share the unit.  The id depends on S as well as on
+                // the unit (S = 2: ids 1-4, S = 4: ids 5-6, S = 8: id 7), so an id always has the same
+                // participants and thread count, whatever the sequence of round sizes.
+                const int bar_id = (role.S == 2 ? 1 : role.S == 4 ? 5 : 7) + role.off;
+                asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "r"(role.S * 32) : "memory");
                 if (role.sp == 0) {
                     for (int sp = 1; sp < role.S; ++sp) {
                         const double* other = mine + (size_t)sp * (ACC1 * 32);
@@ -617,6 +621,9 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
                                 }
                     }
                 }
+                // the writers may not start the next split round's stores into `mine` before warp
+                // sp = 0 has read this round's (the seed warps run ahead, so nothing else holds them)
+                asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "r"(role.S * 32) : "memory");
             }
             if (c.seg >= 0) {
                 // a segment of a left-over round: the sums over its tiles go to the workspace

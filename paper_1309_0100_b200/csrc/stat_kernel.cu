@@ -107,6 +107,15 @@ __global__ void peak_stats_kernel(const double* __restrict__ dchi2, const int64_
     out[2 * j + 1] = i >= 0 ? fap1_of(z, W, A1) : 1.0;
 }
 
+// *flag = 1 if any of v[0..n) is not finite (the caller zeroes the flag first)
+__global__ void __launch_bounds__(kStatThreads) finite_flag_kernel(const double* __restrict__ v, int64_t n, int* flag)
+{
+    bool bad = false;
+    for (int64_t k = (int64_t)blockIdx.x * kStatThreads + threadIdx.x; k < n; k += (int64_t)gridDim.x * kStatThreads)
+        bad |= !isfinite(v[k]);
+    if (bad) *flag = 1;
+}
+
 unsigned stat_grid(int64_t K)
 {
     int64_t b = (K + kStatThreads - 1) / kStatThreads;
@@ -125,6 +134,14 @@ cudaError_t launch_zstat(const double* dchi2, int64_t K, double chi2_base, doubl
 cudaError_t launch_fap1(const double* z, int64_t K, double W, double A1, double* fap_out, cudaStream_t stream)
 {
     fap1_kernel<<<stat_grid(K), kStatThreads, 0, stream>>>(z, K, W, A1, fap_out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_finite_flag(const double* v, int64_t n, int* flag, cudaStream_t stream)
+{
+    cudaError_t e = cudaMemsetAsync(flag, 0, sizeof(int), stream);
+    if (e != cudaSuccess) return e;
+    finite_flag_kernel<<<stat_grid(n), kStatThreads, 0, stream>>>(v, n, flag);
     return cudaGetLastError();
 }
 

@@ -12,6 +12,9 @@ cudaError_t launch_zstat(const double* dchi2, int64_t K, double chi2_base, doubl
 // fap[k] = min(1, A1 W exp(-z[k]) sqrt(z[k]))            (eq. 13 with n = 1)
 cudaError_t launch_fap1(const double* z, int64_t K, double W, double A1, double* fap_out, cudaStream_t stream);
 
+// *flag (device int) = 1 if any of v[0..n) is NaN or infinite, else 0
+cudaError_t launch_finite_flag(const double* v, int64_t n, int* flag, cudaStream_t stream);
+
 // out[0] = T_eff = sqrt(4 pi Var(t)), out[1] = Var(t) (weighted), out[2] = weighted mean of t
 // out[3] = status (0 or FREDEC_EDATA as a double).  One CTA, fixed-order sums.
 cudaError_t launch_bandwidth(const double* t, const double* w, int64_t N, double* out4, cudaStream_t stream);

@@ -167,6 +167,81 @@ def test_subset_fits_large_pool_sampled(fr, p1, n):
     assert np.all(got >= 0.0) and np.all(got <= got[0] * (1 + 1e-12))
 
 
+@pytest.mark.parametrize("n", [20, 22, 25])
+def test_subset_fits_largest_pools_sampled(fr, p1, n):
+    """The pool sizes the paper calls long-but-feasible and "the limit" (PAPER.md:270: 15-20, 25-27;
+    55 Cnc needed n = 25): 2^n fits in one call, sampled masks (+ empty, full, single bits) against
+    the oracle's from-scratch Cholesky."""
+    rng = np.random.Generator(np.random.PCG64(100 + n))
+    N = 800
+    t = np.sort(rng.uniform(0.0, 900.0, N))
+    freqs = np.sort(rng.uniform(0.01, 0.9, n))
+    x = rng.standard_normal(N) + sum(1.2 * np.cos(2 * np.pi * f * t + j) for j, f in enumerate(freqs[::4]))
+    w = rng.uniform(0.5, 2.0, N)
+    got = fr.fredec_subset_fits(t, x, w, freqs)
+    masks = np.unique(np.concatenate([[0, (1 << n) - 1], 1 << np.arange(n), rng.integers(0, 1 << n, 200),
+                                      ((1 << n) - 1) ^ (1 << np.arange(0, n, 5))]))
+    ref = p1.subset_fits(t, x, w, freqs, masks=masks)
+    D = float(np.sum(w * x * x))
+    assert got.shape == (1 << n,)
+    assert np.max(np.abs(got[masks] - ref)) <= 1e-10 * D
+    assert np.all(got >= 0.0) and np.all(got <= got[0] * (1 + 1e-12))
+
+
+def _alias_example_series():
+    """The own series of tests/golden/alias_example.txt (0.9 and 1.1 Hz, gaps aliasing at 0.1 Hz)."""
+    import os
+    cfg = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "alias_example.txt")) as fh:
+        for line in fh:
+            if line.strip() and not line.startswith("#"):
+                k, v = line.split("=")
+                cfg[k.strip()] = float(v)
+    n_per = int(round(cfg["window"] / cfg["dt"]))
+    t = np.concatenate([m * cfg["gap_period"] + cfg["dt"] * np.arange(n_per) for m in range(int(cfg["n_windows"]))])
+    rng = np.random.Generator(np.random.PCG64(294))
+    x = np.cos(2 * np.pi * cfg["f_a"] * t) + np.cos(2 * np.pi * cfg["f_b"] * t + 1.0) + 0.1 * rng.standard_normal(t.size)
+    return t, x, np.ones_like(t)
+
+
+@pytest.mark.parametrize("which", ["rv_like_pool", "alias_comb", "near_duplicates"])
+def test_subset_fits_aliased_pools(fr, p1, which):
+    """Pools as phase 1 really produces them ("will likely contain some aliases"): Q of a
+    subset that holds a frequency and its aliases is badly conditioned, which is where the walk's
+    incrementally updated L^{-1} loses digits.  Pools: (a) the pool the ORACLE's phase 1 finds on the
+    config-2 series (seasonal gaps: yearly alias families); (b) the 0.6 ... 1.4 Hz comb of the alias
+    example; (c) constructed near-duplicates 0.1/T, 1e-3/T and exactly 0 apart.
+    Tolerance as for the benign pools: 1e-10 D, D = <x^2>."""
+    rng = np.random.Generator(np.random.PCG64(7))
+    if which == "rv_like_pool":
+        wl = inputs.config(2)
+        t, x, w, _ = wl.series(0)
+        ref1 = p1.phase1(t, x, w, wl.f0, wl.df, wl.K, max_base=10, k_peaks=32)
+        idx = ref1["pool_idx"][:18]
+        assert idx.size >= 8, "phase 1 should find a pool with aliases on the RV-like series"
+        freqs = wl.f0 + wl.df * idx
+    elif which == "alias_comb":
+        t, x, w = _alias_example_series()
+        freqs = np.array([0.6, 0.7, 0.8, 0.9, 1.0, 1.1, 1.2, 1.3, 1.4])
+    else:
+        t, x, w, _ = inputs.random_series(31, 500, 0, t_span=300.0)
+        T = t.max() - t.min()
+        freqs = np.array([0.05, 0.05 + 0.1 / T, 0.11, 0.11 + 1e-3 / T, 0.2, 0.2, 0.31, 0.31 + 0.03 / T, 0.4])
+    n = freqs.size
+    got = fr.fredec_subset_fits(t, x, w, freqs)
+    masks = np.arange(1 << n) if n <= 10 else np.unique(np.concatenate(
+        [[0, (1 << n) - 1], 1 << np.arange(n), rng.integers(0, 1 << n, 600)]))
+    ref = p1.subset_fits(t, x, w, freqs, masks=masks)
+    D = float(np.sum(w * x * x))
+    err = np.abs(got[masks] - ref)
+    import os
+    os.makedirs("gpurun_out", exist_ok=True)
+    with open(os.path.join("gpurun_out", f"subset_alias_{which}.txt"), "w") as fh:
+        fh.write(f"n={n} masks={masks.size} max|dl|/D={err.max() / D:.3e} at mask {int(masks[np.argmax(err)])}\n")
+    assert np.all(np.isfinite(got)) and np.all(got >= 0.0)
+    assert err.max() <= 1e-10 * D, f"max |dl| / D = {err.max() / D:.3e}"
+
+
 def test_subset_fits_duplicate_frequency_and_errors(fr, p1):
     t, x, w, _ = inputs.random_series(3, 60, 0)
     freqs = np.array([0.2, 0.2, 0.31])
@@ -209,6 +284,23 @@ def test_refine_parity(fr, p1, noise, n):
     f0, l0, it0 = fr.fredec_refine(t, x, w, start, max_iter=0)
     _, l0_ref, _ = p1.refine(t, x, w, start, max_iter=0)
     assert it0 == 0 and np.array_equal(f0, start) and abs(l0 - l0_ref) <= 1e-9 * D
+
+
+def test_non_finite_frequencies_are_data_errors(fr):
+    """freqs must be finite (include/fredec.h): FREDEC_EDATA from host and from device pointers."""
+    import torch
+    t, x, w, _ = inputs.random_series(2, 60, 0)
+    bad = np.array([0.1, np.nan, 0.3])
+    for conv in (lambda a: a, lambda a: torch.from_numpy(a).cuda()):
+        args = [conv(a) for a in (t, x, w)]
+        for fn in (lambda: fr.fredec_trig_averages(*args, conv(bad)),
+                   lambda: fr.fredec_subset_fits(*args, conv(bad)),
+                   lambda: fr.fredec_refine(*args, bad),
+                   lambda: fr.fredec_trig_averages(*args, conv(np.array([np.inf])))):
+            with pytest.raises(fr.FredecError) as e:
+                fn()
+            assert e.value.code == fr.FREDEC_EDATA
+    assert np.all(np.isfinite(fr.fredec_trig_averages(t, x, w, np.array([0.1, 0.2]))))
 
 
 def test_refine_errors(fr):
