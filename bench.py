@@ -162,6 +162,77 @@ def run_cpu_sample(wl, steps: int, warmup: int, threads: int = 0):
                       f"{steps} step(s), OpenMP over frequencies"}
 
 
+def run_small_configs(fr, inputs, dev, stream, peak_nominal, with_oracle: bool):
+    """Configs 1-3 (the tiny, RV-like and residual scans): device-resident step through the C-ABI,
+    per-kernel device times, pairs/s, executed-flop fraction of the FP64 peak, and the CPU oracle's
+    one-core and all-core rates on the same arrays (north_star: "in the same run")."""
+    import torch
+    out = {}
+    for number in (1, 2, 3):
+        wl = inputs.config(number)
+        t, x, w, base = wl.series(0)
+        d_in = [torch.from_numpy(a).to(dev) for a in (t, x, w, base)]
+        z = torch.empty(wl.K, dtype=torch.float64, device=dev)
+        idx = torch.empty(wl.topk, dtype=torch.int64, device=dev)
+
+        def step():
+            return fr.fredec_scan_topk(*d_in, wl.f0, wl.df, wl.K, wl.topk, z_out=z, idx_out=idx)
+
+        for _ in range(3):
+            step()
+        steps = 20
+        kern = {"prep_ms": 0.0, "scan_ms": 0.0, "topk_ms": 0.0}
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record(stream)
+        for _ in range(steps):
+            step()
+            tm = fr.fredec_last_timing()
+            for key in kern:
+                kern[key] += tm[key] / steps
+        b.record(stream)
+        torch.cuda.synchronize()
+        step_ms = a.elapsed_time(b) / steps
+        # the asynchronous form: no host round trip between the steps
+        fr.fredec_set_async(True)
+        try:
+            step()
+            torch.cuda.synchronize()
+            a.record(stream)
+            for _ in range(steps):
+                step()
+            b.record(stream)
+            torch.cuda.synchronize()
+            fr.fredec_last_status()
+        finally:
+            fr.fredec_set_async(False)
+        async_ms = a.elapsed_time(b) / steps
+        F = flops_per_pair(wl.d)
+        rec = {"workload": f"{wl.name}: N={wl.N} x K={wl.K}, d={wl.d}, top-{wl.topk}", "pairs": wl.pairs,
+               "kernel_ms": {"prep": kern["prep_ms"], "scan": kern["scan_ms"], "topk": kern["topk_ms"]},
+               "step_ms": step_ms, "step_ms_async": async_ms,
+               "gpairs_s": wl.pairs / (step_ms * 1e-3) / 1e9,
+               "scan_gpairs_s": wl.pairs / (kern["scan_ms"] * 1e-3) / 1e9,
+               "scan_fraction_of_fp64_peak": wl.pairs * F / (kern["scan_ms"] * 1e-3) / 1e12 / peak_nominal,
+               "flops_per_pair": F, "peaks": idx.cpu().tolist()}
+        if with_oracle:
+            import oracle
+            Ks = wl.K if number < 3 else 40_000          # one core: a bounded sample of config 3 (~10 s)
+            t0 = time.perf_counter()
+            oracle.scan(t, x, w, base, wl.f0, wl.df, Ks, threads=1)
+            one = Ks * wl.N / (time.perf_counter() - t0) / 1e9
+            t0 = time.perf_counter()
+            z_ref = oracle.scan(t, x, w, base, wl.f0, wl.df, wl.K, threads=0)
+            alln = wl.pairs / (time.perf_counter() - t0) / 1e9
+            rec["oracle_gpairs_s"] = {"one_core": one, "all_cores": alln, "cores": oracle.num_threads(),
+                                      "one_core_sample": f"first {Ks} of {wl.K} grid frequencies"}
+            zz = z.cpu().numpy()
+            rec["max_abs_dz_over_max_z"] = float(abs(zz - z_ref).max() / z_ref.max())
+            rec["peaks_equal_oracle"] = idx.cpu().tolist() == oracle.topk(z_ref, wl.topk)[0].tolist()
+        out[f"config{number}"] = rec
+    return out
+
+
 def main_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -218,7 +289,7 @@ def main_ours(args):
     def step_device():
         return fr.fredec_scan_topk(*d_in, f0, wl.df, K, k_req, z_out=z_dev, idx_out=idx_dev)
 
-    peak_tf, _ = fr.fredec_fp64_peak(1 << 17)
+    peak_tf, _ = fr.fredec_bench_fp64(0, 1 << 17)
     sampler = ClockSampler(torch.cuda.current_device()) if rank == 0 else None
 
     for _ in range(max(args.warmup, 3)):
@@ -353,6 +424,8 @@ def main_ours(args):
         "gpu_launches": launches,
         "clocks": clocks,
     }
+    if world == 1 and not args.no_small_configs:
+        line["configs"] = run_small_configs(fr, inputs, dev, stream, peak_nominal, with_oracle=cpu is not None)
     if multi:
         line["multi_series"] = multi
     if cpu:
@@ -364,6 +437,35 @@ def main_ours(args):
     return 0
 
 
+def main_fp64_probe(args):
+    """Prints one JSON line per FP64 roofline probe of include/fredec_bench.h (DFMA-only peak, DMMA-only,
+    DMMA mixed with scalar FP64 instructions): the evidence behind the roofline denominator and behind
+    DESIGN.md's cost of a scalar FP64 instruction next to the MMA stream."""
+    import torch
+    from paper_1309_0100_b200 import build as lib_build
+    lib_build.build()
+    import paper_1309_0100_b200 as fr
+    torch.cuda.set_device(0)
+    fr.fredec_set_stream(torch.cuda.current_stream())
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    mode, base = 0, None
+    while True:
+        name = fr.fredec_bench_fp64_name(mode)
+        if name is None:
+            break
+        best = max(fr.fredec_bench_fp64(mode, 1 << 17 if mode == 0 else 1 << 14)[0] for _ in range(3))
+        rec = {"probe": mode, "name": name, "tflops": best,
+               "frac_of_nominal": best / (sms * FP64_LANES_PER_SM * 2 * 1.965e-3)}
+        if mode >= 1:
+            # SM-sub-partition cycles per DMMA at 1965 MHz with two MMA warps per sub-partition
+            rec["cycles_per_dmma"] = 512.0 * 1.965e9 * sms * 4 / (best * 1e12)
+            base = rec["cycles_per_dmma"] if mode == 1 else base
+            rec["extra_cycles_per_64_dmma_of_a_warp"] = (rec["cycles_per_dmma"] - base) * 64 * 2
+        print(json.dumps(rec))
+        mode += 1
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -372,9 +474,13 @@ def main():
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-multi-series", action="store_true", help="skip the config-5 side measurement")
+    ap.add_argument("--no-small-configs", action="store_true", help="skip the configs 1-3 block")
+    ap.add_argument("--fp64-probe", action="store_true", help="run the FP64 roofline probes and exit")
     args = ap.parse_args()
     if args.steps < 1:
         ap.error("--steps must be >= 1")
+    if args.fp64_probe:
+        return main_fp64_probe(args)
     return main_reference(args) if args.impl == "reference" else main_ours(args)
 
 

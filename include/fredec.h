@@ -22,8 +22,12 @@
  *   - The caller owns every buffer it passes; the library keeps no pointer after return.
  *     Internal workspace is library-owned, grows lazily and is freed by fredec_shutdown().
  *   - Work is enqueued on the stream set by fredec_set_stream() (default: the legacy
- *     default stream).  Every compute entry point returns AFTER its work has completed on
- *     that stream, so that the returned status is final and outputs are ready.
+ *     default stream).  By default every compute entry point returns AFTER its work has
+ *     completed on that stream, so that the returned status is final and outputs are ready.
+ *     fredec_set_async(1) selects the asynchronous form for the scan / top-k calls whose
+ *     pointers are all device pointers: they return once their work is enqueued, outputs are
+ *     ready after the caller's own synchronisation of the stream, and fredec_last_status()
+ *     delivers what the synchronous call would have returned.
  *   - Return value: FREDEC_OK (0) or a count >= 0 on success, a negative FREDEC_E* code
  *     on failure.  Nothing throws, aborts or prints.  On failure outputs are unspecified.
  *   - There is NO CPU fallback: without a usable CUDA device compute calls return
@@ -224,10 +228,52 @@ int fredec_refine(const double* t, const double* x, const double* w, int64_t N,
                   double* freqs, int32_t n, int32_t max_iter, double tol,
                   double* l_out, int32_t* iters_out);
 
+/*
+ * fredec_refine_batched -- the local fit of fredec_refine for T tuples drawn from one pool of n_pool
+ * frequencies, in one call: the table of l_{m,loc} that phase 2 builds for the subsets of the pool
+ * (PAPER.md:214), computed as "many entirely independent instances of the fitting subroutine"
+ * -- one thread block per tuple, all Gauss-Newton iterations on the device.
+ *   t, x, w [N];  pool_freqs [n_pool], finite, 1 <= n_pool <= 25: the start frequencies
+ *   masks [T]     bit j of masks[i] selects pool_freqs[j] for tuple i (0 <= masks[i] < 2^n_pool; the empty
+ *                 tuple is the constant alone); NULL: every tuple is the whole pool.  N >= 3m + 2 for the
+ *                 largest tuple size m (host masks are checked; device masks are not read back, and the
+ *                 requirement is then N >= 3 n_pool + 2)
+ *   max_iter, tol as fredec_refine
+ *   freqs_out [T][n_pool]  refined frequencies of the selected entries, pool_freqs[j] for the others
+ *   l_out [T]              min chi2 at the returned frequencies
+ *   iters_out, status_out [T] int32 (either may be NULL): frequency updates made; 0 or FREDEC_ESINGULAR
+ *                 (singular normal equations, e.g. two equal frequencies in the tuple; l_out is then 0)
+ * Returns the number of tuples whose status is not 0 (so 0 = every fit succeeded), or a negative error
+ * code (FREDEC_EDATA: non-finite frequency or bad t / w).
+ */
+int fredec_refine_batched(const double* t, const double* x, const double* w, int64_t N,
+                          const double* pool_freqs, int32_t n_pool, const int64_t* masks, int64_t T,
+                          int32_t max_iter, double tol,
+                          double* freqs_out, double* l_out, int32_t* iters_out, int32_t* status_out);
+
 /* ----------------------------------------------------------------- runtime control */
 
 /* Stream on which all work is enqueued (a cudaStream_t passed as void*); NULL = default. */
 int fredec_set_stream(void* cuda_stream);
+
+/*
+ * fredec_set_async -- enable != 0: fredec_scan, fredec_scan_batched, fredec_topk, fredec_topk_batched,
+ * fredec_scan_topk and fredec_scan_topk_batched return FREDEC_OK as soon as their work is enqueued on
+ * the library's stream, PROVIDED every data pointer of the call is a device pointer (a call with a host
+ * pointer stays synchronous: the library may keep no host pointer after return).  Argument errors are
+ * still returned at once.  Data errors (FREDEC_EDATA, FREDEC_ESINGULAR) and the peak count are then
+ * obtained with fredec_last_status().  The next compute call resolves a pending one first (their status
+ * buffers are shared), so at most one call is ever pending.  enable == 0 (default): synchronous.
+ */
+int fredec_set_async(int32_t enable);
+
+/*
+ * fredec_last_status -- waits for the pending asynchronous call, if any (synchronises the stream), and
+ * returns the status the synchronous form would have returned: FREDEC_OK or a negative code; *count_out
+ * (may be NULL) receives the number of peaks of series 0 when the call extracted peaks.  Without a
+ * pending call it repeats the status of the last resolved one.
+ */
+int fredec_last_status(int32_t* count_out);
 
 /* Device-side durations (ms, CUDA events on the library's stream) of the kernels of the LAST
  * compute call: out[0] = base orthogonalisation + packing kernel(s), out[1] = scan kernel(s),
@@ -236,11 +282,6 @@ int fredec_last_timing(double out[4]);
 
 /* Number of kernels the LAST compute call launched. */
 int fredec_last_launches(void);
-
-/* Measures the FP64 FMA peak of the current device with a register-resident DFMA-only
- * kernel on all SMs (roofline denominator, not part of the method).  iters = FMAs per
- * thread per chain (>= 1024).  Outputs TFLOP/s (FMA = 2 flops) and kernel ms. */
-int fredec_fp64_peak(int64_t iters, double* tflops_out, double* ms_out);
 
 /* Frees all library-owned device memory, events and staging buffers. */
 int fredec_shutdown(void);

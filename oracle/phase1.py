@@ -105,12 +105,14 @@ def phase1(t, x, w, f0, df, K, fap0=0.05, fap1_thr=0.1, A1=1.0, max_base=10, k_p
             "base_idx": np.array(base_idx, dtype=np.int64)}
 
 
-def subset_fits(t, x, w, freqs, tau: float = 1e-10, masks=None):
+def subset_fits(t, x, w, freqs, tau: float = 1e-10, masks=None, return_pivots: bool = False):
     """PAPER.md:158-175 (section 3) for every subset of the pool `freqs` (the 2^n - 1
     fits of phase 2, here with the frequencies held fixed: l_m(f') of eq. 7):
     g and Q of eqs. 15-16 summed directly, Cholesky Q = L L^T, a = L^{-1} g by forward substitution,
     l = D - |a|^2 (reading G2).  A column whose pivot^2 <= tau * (its diagonal) is dropped (reading S6).
-    Returns l[mask], mask = 0 .. 2^n - 1, bit j selecting freqs[j] (or only for the given masks)."""
+    Returns l[mask], mask = 0 .. 2^n - 1, bit j selecting freqs[j] (or only for the given masks); with
+    return_pivots also the smallest relative pivot^2 / diagonal of each fit (0 when a column was dropped):
+    a diagnostic of the conditioning, about eps / pivot of D is lost to rounding on any FP64 path."""
     t, x, w = (np.asarray(a, dtype=np.float64) for a in (t, x, w))
     n = len(freqs)
     Phi = sinusoid_base(t, freqs)                       # rows 1, cos w_1 t, sin w_1 t, ...
@@ -119,6 +121,7 @@ def subset_fits(t, x, w, freqs, tau: float = 1e-10, masks=None):
     D = np.sum(w * x * x)
     masks = range(1 << n) if masks is None else [int(m) for m in masks]
     out = np.empty(len(masks))
+    pmin = np.ones(len(masks))
     for pos, mask in enumerate(masks):
         idx = [0] + [c for j in range(n) if (mask >> j) & 1 for c in (2 * j + 1, 2 * j + 2)]
         m = len(idx)
@@ -132,8 +135,11 @@ def subset_fits(t, x, w, freqs, tau: float = 1e-10, masks=None):
             if piv2 > tau * Q[idx[i], idx[i]]:
                 L[i, i] = np.sqrt(piv2)
                 a[i] = (g[idx[i]] - L[i, :i] @ a[:i]) / L[i, i]
+                pmin[pos] = min(pmin[pos], piv2 / Q[idx[i], idx[i]])
+            else:
+                pmin[pos] = 0.0
         out[pos] = max(D - a @ a, 0.0)
-    return out
+    return (out, pmin) if return_pivots else out
 
 
 def refine(t, x, w, freqs, max_iter: int = 20, tol: float = 1e-9):

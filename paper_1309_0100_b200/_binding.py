@@ -38,10 +38,14 @@ SIGNATURES = {
     "fredec_subset_fits": (C.c_int, [_P, _P, _P, _I64, _P, _I32, _P]),
     "fredec_refine": (C.c_int, [_P, _P, _P, _I64, _P, _I32, _I32, _F64, C.POINTER(C.c_double),
                                 C.POINTER(C.c_int32)]),
+    "fredec_refine_batched": (C.c_int, [_P, _P, _P, _I64, _P, _I32, _P, _I64, _I32, _F64, _P, _P, _P, _P]),
     "fredec_set_stream": (C.c_int, [_P]),
+    "fredec_set_async": (C.c_int, [_I32]),
+    "fredec_last_status": (C.c_int, [C.POINTER(C.c_int32)]),
     "fredec_last_timing": (C.c_int, [C.POINTER(C.c_double)]),
     "fredec_last_launches": (C.c_int, []),
-    "fredec_fp64_peak": (C.c_int, [_I64, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    "fredec_bench_fp64": (C.c_int, [_I32, _I64, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    "fredec_bench_fp64_name": (C.c_char_p, [_I32]),
     "fredec_shutdown": (C.c_int, []),
     "fredec_strerror": (C.c_char_p, [C.c_int]),
     "fredec_last_cuda_error": (C.c_int, []),
@@ -114,6 +118,18 @@ def fredec_set_stream(stream=None) -> None:
     """stream: None (default stream), an int cudaStream_t, or a torch.cuda.Stream."""
     handle = 0 if stream is None else getattr(stream, "cuda_stream", stream)
     _check(lib().fredec_set_stream(C.c_void_p(int(handle))), "fredec_set_stream")
+
+
+def fredec_set_async(enable: bool) -> None:
+    """Asynchronous form for scan / top-k calls on device pointers; see include/fredec.h."""
+    _check(lib().fredec_set_async(1 if enable else 0), "fredec_set_async")
+
+
+def fredec_last_status() -> int:
+    """Resolves the pending asynchronous call: raises on a data error, else returns the peak count."""
+    count = C.c_int32(0)
+    _check(lib().fredec_last_status(C.byref(count)), "fredec_last_status")
+    return count.value
 
 
 def fredec_scan(t, x, w, base_funcs, f0, df, K, z_out=None):
@@ -286,6 +302,25 @@ def fredec_refine(t, x, w, freqs, max_iter=20, tol=1e-9):
     return f, l.value, it.value
 
 
+def fredec_refine_batched(t, x, w, pool_freqs, masks=None, max_iter=20, tol=1e-9, T=None):
+    """Local multifrequency fits of many tuples of one pool (bit j of masks[i] selects pool_freqs[j];
+    masks=None with T: T copies of the whole pool).  Returns (freqs [T][n_pool], l [T], iters [T] int32,
+    status [T] int32) as numpy arrays."""
+    N, n_pool = int(t.shape[-1]), int(pool_freqs.shape[-1])
+    if masks is not None:
+        masks = np.ascontiguousarray(masks.cpu().numpy() if _is_torch(masks) else masks, dtype=np.int64)
+        T = int(masks.shape[0])
+    T = 1 if T is None else int(T)
+    freqs = np.empty((T, n_pool))
+    l = np.empty(T)
+    iters, status = np.empty(T, dtype=np.int32), np.empty(T, dtype=np.int32)
+    (pt, kt), (px, kx), (pw, kw), (pp, kp) = map(_ptr, (t, x, w, pool_freqs))
+    _check(lib().fredec_refine_batched(pt, px, pw, N, pp, n_pool, None if masks is None else masks.ctypes.data, T,
+                                       int(max_iter), float(tol), freqs.ctypes.data, l.ctypes.data,
+                                       iters.ctypes.data, status.ctypes.data), "fredec_refine_batched")
+    return freqs, l, iters, status
+
+
 def fredec_last_timing() -> dict:
     out = (C.c_double * 4)()
     _check(lib().fredec_last_timing(out), "fredec_last_timing")
@@ -296,11 +331,17 @@ def fredec_last_launches() -> int:
     return int(lib().fredec_last_launches())
 
 
-def fredec_fp64_peak(iters: int = 1 << 16):
-    """(TFLOP/s, ms) of the DFMA-only microbenchmark: the FP64 roofline denominator."""
+def fredec_bench_fp64(mode: int = 0, iters: int = 1 << 16):
+    """(TFLOP/s, ms) of an FP64 roofline probe (include/fredec_bench.h): mode 0 = DFMA only (the FP64
+    FMA peak), modes >= 1 = DMMA loops, see fredec_bench_fp64_name."""
     tf, ms = C.c_double(), C.c_double()
-    _check(lib().fredec_fp64_peak(int(iters), C.byref(tf), C.byref(ms)), "fredec_fp64_peak")
+    _check(lib().fredec_bench_fp64(int(mode), int(iters), C.byref(tf), C.byref(ms)), "fredec_bench_fp64")
     return tf.value, ms.value
+
+
+def fredec_bench_fp64_name(mode: int):
+    name = lib().fredec_bench_fp64_name(int(mode))
+    return None if name is None else name.decode()
 
 
 def fredec_shutdown() -> None:

@@ -26,7 +26,8 @@ def _nvcc() -> str:
 
 def _newest_header() -> float:
     hs = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith(".cuh")]
-    hs += [os.path.join(ROOT, "include", "fredec.h"), os.path.abspath(__file__)]
+    hs += [os.path.join(ROOT, "include", h) for h in os.listdir(os.path.join(ROOT, "include")) if h.endswith(".h")]
+    hs.append(os.path.abspath(__file__))
     return max(os.path.getmtime(h) for h in hs)
 
 

@@ -10,6 +10,7 @@
 #include <cuda_runtime.h>
 
 #include "fredec.h"
+#include "fredec_bench.h"
 #include "peak_kernel.cuh"
 #include "prep_kernel.cuh"
 #include "scan_mma_kernel.cuh"
@@ -81,11 +82,18 @@ struct State {
     cudaEvent_t ev[kNumEvents] = {};
     DevBuf in_t, in_x, in_w, in_base, in_z, out_z, out_idx, out_chi2;
     DevBuf gram, rf, part, p1_base, p1_freq, p1_z, p1_idx, p1_stats, tab, srec, psi, xt, info, ws, red, part_z, part_i, count, sink;
-    HostBuf h_info, h_count, h_flag;
+    HostBuf h_info, h_count, h_flag, h_p1;
     DevBuf flag;
     int last_cuda = 0;
     double timing[4] = {0, 0, 0, 0};
     int launches = 0;
+    // asynchronous form (fredec_set_async): a scan / top-k call whose pointers are all device pointers
+    // returns after enqueueing; its status is resolved by fredec_last_status()
+    bool async_mode = false;
+    bool pending = false;        // a call has been enqueued and not yet resolved
+    bool pend_series = false, pend_topk = false;
+    int64_t pend_B = 0;
+    int last_status = 0, last_count = 0;
 };
 State g;
 
@@ -204,12 +212,16 @@ struct Call {
     int64_t* didx = nullptr;  // device peak indices [B][k]
     int64_t* hidx = nullptr;
     size_t idx_count = 0;
+    bool staged_inputs = false;  // an input was a host pointer (copied through library memory)
 };
+
+int resolve_pending();
 
 int begin_call()
 {
     int rc = ensure_ready();
     if (rc) return rc;
+    if (g.pending) (void)resolve_pending();  // its events and pinned status buffers are about to be reused
     g.launches = 0;
     for (double& v : g.timing) v = 0.0;
     CK(cudaEventRecord(g.ev[0], g.stream));
@@ -270,11 +282,13 @@ int enqueue_series_mma(Call& c, const double* dt, const double* dx, const double
     sp.f0 = f0; sp.df = df;
     sp.n_pass = n_pass;
     sp.grid = (int)(sp.T < (int64_t)g.sm_count ? sp.T : (int64_t)g.sm_count);
-    // ring of (table tile, seeds) slots: 32 observations per slot (two groups of 4 per seed warp)
-    // if at least three slots fit in ~208 KB of shared memory, else 16; as many slots as fit
+    // ring of (table tile, seeds) slots: as many observations per slot (at most 32: two groups of 4
+    // per seed warp) as leave room for three slots in shared memory; short series take 16
+    constexpr size_t kSmemBudget = 221000;  // of the 232448 B a CTA may have: the kernel adds 8 KB behind the ring and ~1.3 KB static
     sp.TI = 32;
-    if ((208 * 1024) / mma_scan_slot_bytes(NB, sp.TI) < 3 || G4 <= 4) sp.TI = 16;
-    sp.NS = (int)((208 * 1024) / mma_scan_slot_bytes(NB, sp.TI));
+    while (sp.TI > 16 && 3 * mma_scan_slot_bytes(NB, sp.TI) > kSmemBudget) sp.TI -= 4;
+    if (G4 <= 4) sp.TI = 16;
+    sp.NS = (int)(kSmemBudget / mma_scan_slot_bytes(NB, sp.TI));
     if (sp.NS > kMmaMaxSlots) sp.NS = kMmaMaxSlots;
     if (sp.NS < 2) return FREDEC_EINVAL;
     sp.ws = nullptr;
@@ -322,6 +336,7 @@ int enqueue_series(Call& c, const double* t, const double* x, const double* w, i
     if ((rc = stage_in(x, BN, g.in_x, &dx))) return rc;
     if ((rc = stage_in(w, BN, g.in_w, &dw))) return rc;
     if ((rc = stage_in(base_funcs, BN * d, g.in_base, &dbase))) return rc;
+    c.staged_inputs = dt != t || dx != x || dw != w || dbase != base_funcs;
 
     if (with_scan) return enqueue_series_mma(c, dt, dx, dw, dbase, B, N, d, f0, df, K, z_out);
 
@@ -375,8 +390,37 @@ int enqueue_topk(Call& c, const double* dz, int64_t B, int64_t K, int32_t k, int
     return FREDEC_OK;
 }
 
-// copies results out, synchronises once, reads statuses; *first_count = peaks of series 0
-int finish_call(Call& c, int* first_count)
+// Waits for the enqueued call and reads its statuses: the first series status that is not 0, else 0;
+// g.last_count = peaks of series 0.
+int resolve_pending()
+{
+    if (!g.pending) return g.last_status;
+    g.pending = false;
+    g.last_status = FREDEC_ECUDA;
+    g.last_count = 0;
+    CK(cudaStreamSynchronize(g.stream));
+    if (g.pend_series) {
+        g.timing[0] = ev_ms(1, 2);
+        g.timing[1] = ev_ms(2, 3);
+    }
+    if (g.pend_topk) g.timing[2] = ev_ms(4, 5);
+    g.timing[3] = ev_ms(0, 6);
+    g.last_status = FREDEC_OK;
+    if (g.pend_series) {
+        const SeriesInfo* hi = static_cast<const SeriesInfo*>(g.h_info.p);
+        for (int64_t b = 0; b < g.pend_B; ++b)
+            if (hi[b].status != 0) {
+                g.last_status = hi[b].status;
+                break;
+            }
+    }
+    if (g.pend_topk && g.last_status == FREDEC_OK) g.last_count = static_cast<const int*>(g.h_count.p)[0];
+    return g.last_status;
+}
+
+// Copies results out and either synchronises and reads the statuses (*first_count = peaks of series 0),
+// or -- `defer`, or the asynchronous mode with nothing to copy to the host -- leaves the call pending.
+int finish_call(Call& c, int* first_count, bool defer = false)
 {
     cudaStream_t st = g.stream;
     if (c.hz) CK(cudaMemcpyAsync(c.hz, c.dz, c.z_count * 8, cudaMemcpyDeviceToHost, st));
@@ -386,20 +430,14 @@ int finish_call(Call& c, int* first_count)
     if (c.has_topk)
         CK(cudaMemcpyAsync(g.h_count.p, g.count.p, (size_t)c.B * sizeof(int), cudaMemcpyDeviceToHost, st));
     CK(cudaEventRecord(g.ev[6], st));
-    CK(cudaStreamSynchronize(st));
-    if (c.has_series) {
-        g.timing[0] = ev_ms(1, 2);
-        g.timing[1] = ev_ms(2, 3);
-    }
-    if (c.has_topk) g.timing[2] = ev_ms(4, 5);
-    g.timing[3] = ev_ms(0, 6);
-    if (c.has_series) {
-        const SeriesInfo* hi = static_cast<const SeriesInfo*>(g.h_info.p);
-        for (int64_t b = 0; b < c.B; ++b)
-            if (hi[b].status != 0) return hi[b].status;
-    }
-    if (c.has_topk && first_count) *first_count = static_cast<const int*>(g.h_count.p)[0];
-    return FREDEC_OK;
+    g.pending = true;
+    g.pend_series = c.has_series;
+    g.pend_topk = c.has_topk;
+    g.pend_B = c.B;
+    if (defer || (g.async_mode && !c.hz && !c.hidx && !c.staged_inputs)) return FREDEC_OK;
+    const int rc = resolve_pending();
+    if (first_count) *first_count = g.last_count;
+    return rc;
 }
 
 int check_grid_args(double f0, double df, int64_t K)
@@ -416,7 +454,8 @@ int check_topk_args(int64_t B, int64_t K, int32_t k)
 }
 
 int do_scan(const double* t, const double* x, const double* w, int64_t B, int64_t N, const double* base_funcs,
-            int32_t d, double f0, double df, int64_t K, double* z_out, int32_t k, int64_t* idx_out, bool want_topk)
+            int32_t d, double f0, double df, int64_t K, double* z_out, int32_t k, int64_t* idx_out, bool want_topk,
+            bool defer = false)
 {
     int rc = check_series_args(t, x, w, B, N, base_funcs, d);
     if (rc) return rc;
@@ -432,7 +471,7 @@ int do_scan(const double* t, const double* x, const double* w, int64_t B, int64_
     if ((rc = enqueue_series(c, t, x, w, B, N, base_funcs, d, f0, df, K, z_out, true))) return rc;
     if (want_topk && (rc = enqueue_topk(c, c.dz, B, K, k, idx_out))) return rc;
     int count = 0;
-    if ((rc = finish_call(c, &count))) return rc;
+    if ((rc = finish_call(c, &count, defer))) return rc;
     return (want_topk && B == 1) ? count : FREDEC_OK;
 }
 
@@ -469,6 +508,7 @@ int do_topk(const double* z, int64_t B, int64_t K, int32_t k, int64_t* idx_out, 
     const double* dz;
     if ((rc = stage_in(z, (size_t)B * K, g.in_z, &dz))) return rc;
     Call c;
+    c.staged_inputs = dz != z;
     if ((rc = enqueue_topk(c, dz, B, K, k, idx_out))) return rc;
     return finish_call(c, first_count);
 }
@@ -634,8 +674,10 @@ int fredec_phase1(const double* t, const double* x, const double* w, int64_t N, 
     CK(g.p1_z.reserve((size_t)K * 8));
     CK(g.p1_idx.reserve((size_t)k_peaks * 8));
     CK(g.p1_stats.reserve((size_t)k_peaks * 16));
-    std::vector<double> base_f, stats(2 * (size_t)k_peaks);
-    std::vector<int64_t> idx((size_t)k_peaks);
+    CK(g.h_p1.reserve((size_t)k_peaks * 24));  // pinned: peak indices, then (z, FAP) pairs
+    int64_t* idx = static_cast<int64_t*>(g.h_p1.p);
+    double* stats = reinterpret_cast<double*>(idx + k_peaks);
+    std::vector<double> base_f;
     std::vector<PoolEntry> pool;
     int launches = 1;
     *n_base_out = 0;
@@ -646,19 +688,23 @@ int fredec_phase1(const double* t, const double* x, const double* w, int64_t N, 
         if (NH <= 0.0 || N < (int64_t)d + 3) break;
         if (m > 0) CK(cudaMemcpyAsync(g.p1_freq.p, base_f.data(), (size_t)m * 8, cudaMemcpyHostToDevice, st));
         CK(launch_sin_base(dt, N, g.p1_freq.as<double>(), m, g.p1_base.as<double>(), st));
-        const int count = do_scan(dt, dx, dw, 1, N, g.p1_base.as<double>(), d, f0, df, K, g.p1_z.as<double>(), k_peaks,
-                                  g.p1_idx.as<int64_t>(), true);
+        // one host round trip per iteration: the scan and the peak search are enqueued without a
+        // synchronisation, the peak statistics read chi2_base from device memory, and the statuses,
+        // indices and statistics come back together
+        int rc1 = do_scan(dt, dx, dw, 1, N, g.p1_base.as<double>(), d, f0, df, K, g.p1_z.as<double>(), k_peaks,
+                          g.p1_idx.as<int64_t>(), true, true);
         launches += 1 + g.launches;
-        if (count < 0) return count;
+        if (rc1 < 0) return rc1;
+        CK(launch_peak_stats(g.p1_z.as<double>(), g.p1_idx.as<int64_t>(), k_peaks, g.info.as<SeriesInfo>(), NH, W, A1,
+                             g.p1_stats.as<double>(), st));
+        launches += 1;
+        CK(cudaMemcpyAsync(idx, g.p1_idx.p, (size_t)k_peaks * 8, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(stats, g.p1_stats.p, (size_t)k_peaks * 16, cudaMemcpyDeviceToHost, st));
+        if ((rc1 = resolve_pending()) < 0) return rc1;
+        const int count = g.last_count;
         if (count == 0) break;
         const double chi2_base = static_cast<const SeriesInfo*>(g.h_info.p)[0].chi2_base;
         if (!(chi2_base > 0.0)) break;  // the base model already fits exactly
-        CK(launch_peak_stats(g.p1_z.as<double>(), g.p1_idx.as<int64_t>(), k_peaks, chi2_base, NH, W, A1,
-                             g.p1_stats.as<double>(), st));
-        launches += 1;
-        CK(cudaMemcpyAsync(idx.data(), g.p1_idx.p, (size_t)k_peaks * 8, cudaMemcpyDeviceToHost, st));
-        CK(cudaMemcpyAsync(stats.data(), g.p1_stats.p, (size_t)k_peaks * 16, cudaMemcpyDeviceToHost, st));
-        CK(cudaStreamSynchronize(st));
         const double z_top = stats[0], fap_top = stats[1];
         if (fap_top > fap0) break;
         for (int j = 0; j < count; ++j) {
@@ -748,73 +794,91 @@ int fredec_subset_fits(const double* t, const double* x, const double* w, int64_
     return flag_status();
 }
 
-int fredec_refine(const double* t, const double* x, const double* w, int64_t N, double* freqs, int32_t n,
-                  int32_t max_iter, double tol, double* l_out, int32_t* iters_out)
+int fredec_refine_batched(const double* t, const double* x, const double* w, int64_t N, const double* pool_freqs,
+                          int32_t n_pool, const int64_t* masks, int64_t T, int32_t max_iter, double tol,
+                          double* freqs_out, double* l_out, int32_t* iters_out, int32_t* status_out)
 {
-    if (!t || !x || !w || !freqs || !l_out || n < 1 || n > 25 || N < 3 * (int64_t)n + 2) return FREDEC_EINVAL;
-    if (max_iter < 0 || !(tol > 0.0) || on_device(l_out) || (iters_out && on_device(iters_out))) return FREDEC_EINVAL;
+    if (!t || !x || !w || !pool_freqs || !freqs_out || !l_out || n_pool < 1 || n_pool > 25 || T < 1 ||
+        T > 0x7fffffff)
+        return FREDEC_EINVAL;
+    if (max_iter < 0 || !(tol > 0.0)) return FREDEC_EINVAL;
     int rc = begin_call();
     if (rc) return rc;
     cudaStream_t st = g.stream;
-    const double *dt, *dx, *dw;
+    // the largest tuple sizes the shared memory and the N >= 3m + 2 requirement; masks on the device are
+    // not read back: the whole pool is then the bound
+    int m_max = n_pool;
+    if (masks && !on_device(masks)) {
+        m_max = 0;
+        for (int64_t i = 0; i < T; ++i) {
+            if (masks[i] < 0 || masks[i] >= ((int64_t)1 << n_pool)) return FREDEC_EINVAL;
+            int c = 0;
+            for (int j = 0; j < n_pool; ++j) c += (int)((masks[i] >> j) & 1);
+            m_max = c > m_max ? c : m_max;
+        }
+    }
+    if (N < 3 * (int64_t)m_max + 2) return FREDEC_EINVAL;
+    const double *dt, *dx, *dw, *dpool;
+    const int64_t* dmask;
     if ((rc = stage_in(t, (size_t)N, g.in_t, &dt))) return rc;
     if ((rc = stage_in(x, (size_t)N, g.in_x, &dx))) return rc;
     if ((rc = stage_in(w, (size_t)N, g.in_w, &dw))) return rc;
-    double bw[4];
-    if ((rc = device_bandwidth(dt, dw, N, bw))) return rc;
-    const double T_eff = bw[0], t0 = bw[2];
-    if (!(T_eff > 0.0)) return FREDEC_EDATA;
-    const int lin = 2 * n + 1, full = 3 * n + 1;
-    CK(g.p1_base.reserve((size_t)full * N * 8));
-    CK(g.p1_freq.reserve((size_t)n * 8));
-    CK(g.gram.reserve((size_t)(full + 1) * (full + 1) * 8));
-    CK(g.rf.reserve((size_t)(full + n + 4) * 8));
-    double* dfreq = g.p1_freq.as<double>();
-    double* rows = g.p1_base.as<double>();
-    double* theta = g.rf.as<double>();   // [full]
-    double* dstep = theta + full;        // [n]
-    double* out2 = dstep + n;            // [2] linear fit, [2] Gauss-Newton step
-    const bool freqs_dev = on_device(freqs);
-    CK(cudaMemcpyAsync(dfreq, freqs, (size_t)n * 8, freqs_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
-    if ((rc = enqueue_finite_check(dfreq, n))) return rc;
-    CK(cudaStreamSynchronize(st));
-    if ((rc = flag_status())) return rc;
-    std::vector<double> hstep((size_t)n);
-    double hout[4];
-    int iters = 0, launches = 1;
-    bool converged = max_iter == 0;
-    while (true) {
-        // linear fit at the current frequencies (eq. 14)
-        CK(launch_model_rows(dt, N, t0, dfreq, n, nullptr, rows, st));
-        CK(launch_gram(rows, dx, dw, N, lin, g.gram.as<double>(), st));
-        CK(launch_chol_solve(g.gram.as<double>(), lin, theta, out2, st));
-        launches += 3;
-        if (converged || iters == max_iter) break;
-        // quadratic model in (theta, f) and its step (eq. 17)
-        CK(launch_model_rows(dt, N, t0, dfreq, n, theta, rows, st));
-        CK(launch_gram(rows, dx, dw, N, full, g.gram.as<double>(), st));
-        CK(launch_gn_step(g.gram.as<double>(), n, theta, 0.5 / T_eff, dstep, out2 + 2, st));
-        CK(launch_axpy_small(dfreq, dstep, n, st));
-        launches += 4;
-        CK(cudaMemcpyAsync(hstep.data(), dstep, (size_t)n * 8, cudaMemcpyDeviceToHost, st));
-        CK(cudaMemcpyAsync(hout, out2, 32, cudaMemcpyDeviceToHost, st));
-        CK(cudaStreamSynchronize(st));
-        if (hout[1] != 0.0 || hout[3] != 0.0) return FREDEC_ESINGULAR;
-        ++iters;
-        double worst = 0.0;
-        for (int k = 0; k < n; ++k) worst = std::fmax(worst, std::fabs(hstep[k]));
-        converged = worst * T_eff <= tol;
-    }
-    CK(cudaMemcpyAsync(hout, out2, 16, cudaMemcpyDeviceToHost, st));
-    CK(cudaMemcpyAsync(freqs, dfreq, (size_t)n * 8, freqs_dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
+    if ((rc = stage_in(pool_freqs, (size_t)n_pool, g.p1_freq, &dpool))) return rc;
+    if ((rc = stage_in(masks, masks ? (size_t)T : 0, g.in_base, &dmask))) return rc;
+    double *dfo, *hfo, *dlo, *hlo;
+    if ((rc = stage_out(freqs_out, (size_t)T * n_pool, g.out_z, &dfo, &hfo))) return rc;
+    if ((rc = stage_out(l_out, (size_t)T, g.rf, &dlo, &hlo))) return rc;
+    // iteration counts and statuses always go through library buffers (they are read here for the return code)
+    CK(g.part_i.reserve((size_t)T * 2 * sizeof(int32_t)));
+    int32_t* dit = g.part_i.as<int32_t>();
+    int32_t* dstat = dit + T;
+    CK(g.h_count.reserve((size_t)T * 2 * sizeof(int32_t)));
+    if ((rc = enqueue_finite_check(dpool, n_pool))) return rc;
+    CK(g.sink.reserve(64));
+    CK(launch_bandwidth(dt, dw, N, g.sink.as<double>(), st));
+    RefineParams rp;
+    rp.t = dt; rp.x = dx; rp.w = dw; rp.bw = g.sink.as<double>(); rp.pool = dpool; rp.masks = dmask;
+    rp.freqs_out = dfo; rp.l_out = dlo; rp.iters_out = dit; rp.status_out = dstat;
+    rp.N = N; rp.n_pool = n_pool; rp.max_iter = max_iter; rp.tol = tol;
+    CK(cudaEventRecord(g.ev[2], st));
+    CK(launch_refine_batched(rp, T, m_max, st));
+    CK(cudaEventRecord(g.ev[3], st));
+    g.launches += 3;
+    if (hfo) CK(cudaMemcpyAsync(hfo, dfo, (size_t)T * n_pool * 8, cudaMemcpyDeviceToHost, st));
+    if (hlo) CK(cudaMemcpyAsync(hlo, dlo, (size_t)T * 8, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(g.h_count.p, dit, (size_t)T * 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    if (iters_out && on_device(iters_out))
+        CK(cudaMemcpyAsync(iters_out, dit, (size_t)T * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+    if (status_out && on_device(status_out))
+        CK(cudaMemcpyAsync(status_out, dstat, (size_t)T * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
     CK(cudaEventRecord(g.ev[6], st));
     CK(cudaStreamSynchronize(st));
+    g.timing[1] = ev_ms(2, 3);
     g.timing[3] = ev_ms(0, 6);
-    g.launches = launches;
-    if (hout[1] != 0.0) return FREDEC_ESINGULAR;
-    *l_out = hout[0];
+    if ((rc = flag_status())) return rc;
+    const int32_t* hit = static_cast<const int32_t*>(g.h_count.p);
+    const int32_t* hstat = hit + T;
+    if (iters_out && !on_device(iters_out)) std::memcpy(iters_out, hit, (size_t)T * sizeof(int32_t));
+    if (status_out && !on_device(status_out)) std::memcpy(status_out, hstat, (size_t)T * sizeof(int32_t));
+    int failed = 0;
+    for (int64_t i = 0; i < T; ++i) {
+        if (hstat[i] == FREDEC_EDATA) return FREDEC_EDATA;
+        failed += hstat[i] != 0;
+    }
+    return failed;
+}
+
+int fredec_refine(const double* t, const double* x, const double* w, int64_t N, double* freqs, int32_t n,
+                  int32_t max_iter, double tol, double* l_out, int32_t* iters_out)
+{
+    if (!freqs || !l_out || on_device(l_out) || (iters_out && on_device(iters_out))) return FREDEC_EINVAL;
+    if (n < 1 || n > 25 || N < 3 * (int64_t)n + 2) return FREDEC_EINVAL;
+    // one tuple: the whole "pool"; the refined frequencies overwrite the start values
+    int32_t status = 0, iters = 0;
+    const int rc = fredec_refine_batched(t, x, w, N, freqs, n, nullptr, 1, max_iter, tol, freqs, l_out, &iters, &status);
+    if (rc < 0) return rc;
     if (iters_out) *iters_out = iters;
-    return FREDEC_OK;
+    return status == 0 ? FREDEC_OK : status;
 }
 
 int fredec_set_stream(void* cuda_stream)
@@ -823,32 +887,63 @@ int fredec_set_stream(void* cuda_stream)
     return FREDEC_OK;
 }
 
+int fredec_set_async(int32_t enable)
+{
+    if (g.pending) (void)resolve_pending();
+    g.async_mode = enable != 0;
+    return FREDEC_OK;
+}
+
+int fredec_last_status(int32_t* count_out)
+{
+    const int rc = resolve_pending();
+    if (count_out) *count_out = rc == FREDEC_OK ? g.last_count : 0;
+    return rc;
+}
+
 int fredec_last_timing(double out[4])
 {
     if (!out) return FREDEC_EINVAL;
+    if (g.pending) (void)resolve_pending();
     for (int i = 0; i < 4; ++i) out[i] = g.timing[i];
     return FREDEC_OK;
 }
 
 int fredec_last_launches(void) { return g.launches; }
 
-int fredec_fp64_peak(int64_t iters, double* tflops_out, double* ms_out)
+int fredec_bench_fp64(int32_t mode, int64_t iters, double* tflops_out, double* ms_out)
 {
-    if (iters < 1024 || !tflops_out) return FREDEC_EINVAL;
+    if (!tflops_out || mode < 0 || mode > dmma_probe_count()) return FREDEC_EINVAL;
+    if (mode == 0 ? iters < 1024 : (iters < 64 || iters % 4 != 0)) return FREDEC_EINVAL;
     int rc = ensure_ready();
     if (rc) return rc;
     CK(g.sink.reserve(64));
-    const int blocks = g.sm_count * 8;  // 2048 threads per SM
     cudaStream_t st = g.stream;
-    CK(launch_dfma(1024, blocks, g.sink.as<double>(), st));  // warm-up
-    CK(cudaEventRecord(g.ev[0], st));
-    CK(launch_dfma(iters, blocks, g.sink.as<double>(), st));
+    double flops;
+    if (mode == 0) {
+        const int blocks = g.sm_count * 8;  // 2048 threads per SM
+        CK(launch_dfma(1024, blocks, g.sink.as<double>(), st));  // warm-up
+        CK(cudaEventRecord(g.ev[0], st));
+        CK(launch_dfma(iters, blocks, g.sink.as<double>(), st));
+        flops = dfma_flops(iters, blocks);
+    } else {
+        CK(launch_dmma_probe(mode - 1, 64, g.sm_count, g.sink.as<double>(), st));
+        CK(cudaEventRecord(g.ev[0], st));
+        CK(launch_dmma_probe(mode - 1, iters, g.sm_count, g.sink.as<double>(), st));
+        flops = dmma_probe_flops(iters, g.sm_count);
+    }
     CK(cudaEventRecord(g.ev[1], st));
     CK(cudaStreamSynchronize(st));
     const double ms = ev_ms(0, 1);
-    *tflops_out = ms > 0.0 ? dfma_flops(iters, blocks) / (ms * 1e-3) * 1e-12 : 0.0;
+    *tflops_out = ms > 0.0 ? flops / (ms * 1e-3) * 1e-12 : 0.0;
     if (ms_out) *ms_out = ms;
     return FREDEC_OK;
+}
+
+const char* fredec_bench_fp64_name(int32_t mode)
+{
+    if (mode == 0) return "dfma only, 2048 threads per SM";
+    return dmma_probe_name(mode - 1);
 }
 
 int fredec_shutdown(void)
@@ -858,6 +953,7 @@ int fredec_shutdown(void)
     for (DevBuf* b : bufs) b->release();
     g.h_info.release();
     g.h_flag.release();
+    g.h_p1.release();
     g.flag.release();
     g.h_count.release();
     if (g.ready)

@@ -1,6 +1,6 @@
 // prep_kernel.cu -- steps a1-a3 of the scan: validate, centre, orthogonalise the base
-// model (prep_kernel, one CTA per series), per-observation table and seed records
-// (table_kernel).  Once per scan.
+// model (prep_kernel, one thread-block cluster per series), per-observation table and seed
+// records (table_kernel).  Once per scan.
 //
 // Generalises the normalisations of PAPER.md:193-197 (eq. 18: <1> = 1, <x> = 0, ...) to an
 // arbitrary linear base model: the base functions are replaced by functions psi_j that are
@@ -8,20 +8,59 @@
 // system of PAPER.md:165-175 (eqs. 15, 16; Cholesky solve) has an identity leading block and
 // collapses to the 2x2 Schur complement the scan kernel solves per frequency.
 //
-// Orthogonalisation is modified Gram-Schmidt applied twice ("twice is enough"), in the
-// weighted inner product <u v> = sum_i w_i u_i v_i, with deterministic (fixed-order)
-// block reductions.
+// Orthogonalisation = Cholesky QR applied twice.  One pass: the whole weighted Gram matrix of
+// (phi_0 .. phi_{d-1}, x) in ONE sweep over the observations (register tiles of 4 x 4 entries per
+// warp), Cholesky G = L L^T in shared memory with x carried as the last row (that row
+// becomes a = L^{-1} g), then psi = L^{-1} phi and x' = x - sum_j a_j psi_j by one forward
+// substitution per observation.  The first pass leaves an orthogonality error of eps x cond(G); the
+// second pass, on the already nearly orthonormal functions, removes it ("twice is enough").  This
+// is O(1) sweeps over the data where Gram-Schmidt needs O(d^2) dependent reductions.
+//
+// A series is shared by the C CTAs of a thread-block cluster (C = 1 for short series): each CTA
+// owns a contiguous slice of the observations, the partial Gram matrices (and the scalars of a1)
+// are added over the cluster through distributed shared memory in rank order, and every CTA then
+// factors the same matrix.  All orders are fixed: results are bitwise reproducible.
+#include <cooperative_groups.h>
+
 #include "prep_kernel.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace fredec {
 
 namespace {
 
-constexpr int kPrepThreadsMax = 1024;  // one long series: as many threads as a CTA can have
-constexpr int kPrepThreadsMin = 256;   // many short series: several CTAs per SM
+constexpr int kPrepThreads = 256;
+constexpr int kPrepWarps = kPrepThreads / 32;
+constexpr int kPrepMaxCluster = 8;
+constexpr int kGramTile = 4;       // a warp accumulates a 4 x 4 block of Gram entries
+constexpr int kGramMinSplit = 64;  // observations per warp at least, when a tile's sweep is split between warps
+
+// Shared-memory layout of the prep kernel (doubles), M = d + 1 columns (the base functions and x).
+struct PrepSmem {
+    int M, LD, tiles, splits;
+    size_t part, gram, chol, diag0, stash, scal, total;  // offsets in doubles; total in bytes
+};
+__host__ __device__ inline PrepSmem prep_smem(int d, int splits)
+{
+    PrepSmem L;
+    L.M = d + 1;
+    L.LD = L.M | 1;  // odd leading dimension: rows fall on different banks
+    const int tm = (L.M + kGramTile - 1) / kGramTile;
+    L.tiles = tm * (tm + 1) / 2;
+    L.splits = splits;
+    size_t o = 0;
+    L.part = o;  o += (size_t)splits * L.tiles * 16;   // per (split, tile): a 4 x 4 block
+    L.gram = o;  o += (size_t)L.M * L.LD;              // this CTA's partial Gram matrix (read by the cluster)
+    L.chol = o;  o += (size_t)L.M * L.LD;              // the cluster's Gram matrix, factored in place
+    L.diag0 = o; o += L.M;
+    L.stash = o; o += (size_t)d * kPrepThreads;        // forward substitution: psi_m of the thread's observation
+    L.scal = o;  o += 16;
+    L.total = o * sizeof(double);
+    return L;
+}
 
 // Fixed-order block sum, result broadcast to all threads.  `red` = 32 doubles of smem.
-template <int TH>
 __device__ double block_sum(double v, double* red)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -30,13 +69,12 @@ __device__ double block_sum(double v, double* red)
     __syncthreads();  // protect `red` from the previous call's readers
     if (lane == 0) red[wid] = v;
     __syncthreads();
-    double r = (lane < (TH >> 5)) ? red[lane] : 0.0;
+    double r = (lane < kPrepWarps) ? red[lane] : 0.0;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) r += __shfl_xor_sync(0xffffffffu, r, o);
     return r;
 }
 
-template <int TH>
 __device__ double block_min(double v, double* red)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -45,27 +83,163 @@ __device__ double block_min(double v, double* red)
     __syncthreads();
     if (lane == 0) red[wid] = v;
     __syncthreads();
-    double r = (lane < (TH >> 5)) ? red[lane] : v;
+    double r = (lane < kPrepWarps) ? red[lane] : v;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) r = fmin(r, __shfl_xor_sync(0xffffffffu, r, o));
     return r;
 }
 
-// <u v> over the series (u may alias v).
-template <int TH>
-__device__ double wdot(const double* __restrict__ w, const double* u, const double* v, int64_t N, double* red)
+// Partial Gram matrix of the columns (rows[0..d-1], xrow) over the observations [i0, i1) of the series:
+// gram[a][b] (a >= b within the tiles of the lower block triangle) = sum_i w_i col_a(i) col_b(i).
+// Work item = (tile, split); a warp sweeps its share of the slice with the lanes striding over the
+// observations and adds the 16 entries over the lanes; the splits are added in fixed order.
+__device__ void gram_partial(const PrepSmem& L, double* sm, const double* __restrict__ w, const double* rows,
+                             const double* xrow, int64_t N, int d, int64_t i0, int64_t i1)
 {
-    double acc = 0.0;
-    for (int64_t i = threadIdx.x; i < N; i += TH) acc = fma(w[i] * u[i], v[i], acc);
-    return block_sum<TH>(acc, red);
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int M = L.M;
+    double* part = sm + L.part;
+    const int64_t len = i1 - i0, per = (len + L.splits - 1) / L.splits;
+    for (int item = wid; item < L.tiles * L.splits; item += kPrepWarps) {
+        const int tile = item % L.tiles, split = item / L.tiles;
+        int ta = 0;
+        while ((ta + 1) * (ta + 2) / 2 <= tile) ++ta;  // tile = ta (ta + 1) / 2 + tb, tb <= ta
+        const int tb = tile - ta * (ta + 1) / 2;
+        const double* pa[kGramTile];
+        const double* pb[kGramTile];
+#pragma unroll
+        for (int j = 0; j < kGramTile; ++j) {
+            const int ca = ta * kGramTile + j, cb = tb * kGramTile + j;
+            pa[j] = ca < d ? rows + (int64_t)ca * N : (ca == d ? xrow : nullptr);
+            pb[j] = cb < d ? rows + (int64_t)cb * N : (cb == d ? xrow : nullptr);
+        }
+        double acc[kGramTile][kGramTile];
+#pragma unroll
+        for (int j = 0; j < kGramTile; ++j)
+#pragma unroll
+            for (int k = 0; k < kGramTile; ++k) acc[j][k] = 0.0;
+        const int64_t s0 = i0 + split * per, s1 = min(i1, s0 + per);
+        for (int64_t i = s0 + lane; i < s1; i += 32) {
+            const double wi = w[i];
+            double va[kGramTile], vb[kGramTile];
+#pragma unroll
+            for (int j = 0; j < kGramTile; ++j) {
+                va[j] = pa[j] ? wi * pa[j][i] : 0.0;
+                vb[j] = pb[j] ? pb[j][i] : 0.0;
+            }
+#pragma unroll
+            for (int j = 0; j < kGramTile; ++j)
+#pragma unroll
+                for (int k = 0; k < kGramTile; ++k) acc[j][k] = fma(va[j], vb[k], acc[j][k]);
+        }
+#pragma unroll
+        for (int j = 0; j < kGramTile; ++j)
+#pragma unroll
+            for (int k = 0; k < kGramTile; ++k) {
+                double v = acc[j][k];
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                if (lane == 0) part[((size_t)split * L.tiles + tile) * 16 + j * kGramTile + k] = v;
+            }
+    }
+    __syncthreads();
+    double* gram = sm + L.gram;
+    for (int e = threadIdx.x; e < L.tiles * 16; e += kPrepThreads) {
+        const int tile = e / 16, j = (e % 16) / kGramTile, k = e % kGramTile;
+        int ta = 0;
+        while ((ta + 1) * (ta + 2) / 2 <= tile) ++ta;
+        const int tb = tile - ta * (ta + 1) / 2;
+        const int a = ta * kGramTile + j, b = tb * kGramTile + k;
+        if (a < M && b <= a) {
+            double v = 0.0;
+            for (int sp = 0; sp < L.splits; ++sp) v += part[((size_t)sp * L.tiles + tile) * 16 + j * kGramTile + k];
+            gram[a * L.LD + b] = v;
+        }
+    }
 }
 
-template <int TH>
-__global__ void __launch_bounds__(TH) prep_kernel(PrepParams p)
+// chol = sum over the cluster's CTAs, in rank order, of their partial Gram matrices (lower triangles).
+__device__ void gram_cluster_sum(const PrepSmem& L, double* sm, cg::cluster_group& cluster)
 {
+    cluster.sync();  // every CTA's partial matrix is written
+    const int M = L.M, C = (int)cluster.num_blocks();
+    double* chol = sm + L.chol;
+    for (int e = threadIdx.x; e < M * M; e += kPrepThreads) {
+        const int a = e / M, b = e % M;
+        if (b > a) continue;
+        double v = 0.0;
+        for (int r = 0; r < C; ++r) v += cluster.map_shared_rank(sm + L.gram, r)[a * L.LD + b];
+        chol[a * L.LD + b] = v;
+        if (a == b) sm[L.diag0 + a] = v;
+    }
+    cluster.sync();  // all remote reads done before anyone overwrites its partial matrix
+}
+
+// In-place Cholesky of the leading d x d block of chol (lower triangle) with row d (the column x) carried
+// along as a right-hand side: afterwards chol[i][j] = L[i][j], chol[d][j] = a_j = (L^{-1} g)_j.
+// Returns false when a pivot^2 <= tau x its original diagonal (dependent base functions, S6b).
+__device__ bool chol_with_x(const PrepSmem& L, double* sm, int d, double tau, int* flag)
+{
+    double* S = sm + L.chol;
+    const double* diag0 = sm + L.diag0;
+    const int LD = L.LD, tid = threadIdx.x;
+    if (tid == 0) *flag = 0;
+    __syncthreads();
+    for (int j = 0; j < d; ++j) {
+        const double piv = S[j * LD + j];
+        if (!(piv > tau * diag0[j])) {  // uniform across the CTA
+            if (tid == 0) *flag = 1;
+            break;
+        }
+        const double ljj = sqrt(piv), inv = 1.0 / ljj;
+        __syncthreads();
+        for (int i = j + tid; i <= d; i += kPrepThreads) S[i * LD + j] = i == j ? ljj : S[i * LD + j] * inv;
+        __syncthreads();
+        const int rows = d - j;  // rows j+1 .. d, columns j+1 .. min(row, d-1)
+        for (int e = tid; e < rows * rows; e += kPrepThreads) {
+            const int i = j + 1 + e / rows, k = j + 1 + e % rows;
+            if (k <= i && k < d) S[i * LD + k] = fma(-S[i * LD + j], S[k * LD + j], S[i * LD + k]);
+        }
+        __syncthreads();
+    }
+    __syncthreads();
+    return *flag == 0;
+}
+
+// psi_j(i) = (phi_j(i) - sum_{m<j} L[j][m] psi_m(i)) / L[j][j],  x'(i) = x(i) - sum_j a_j psi_j(i), one
+// thread per observation of [i0, i1); src / xsrc may alias dst / xdst (a thread touches its own column only).
+__device__ void apply_factor(const PrepSmem& L, double* sm, int d, const double* src, const double* xsrc, double* dst,
+                             double* xdst, int64_t N, int64_t i0, int64_t i1)
+{
+    const double* S = sm + L.chol;
+    double* stash = sm + L.stash + threadIdx.x;
+    const int LD = L.LD;
+    for (int64_t i = i0 + threadIdx.x; i < i1; i += kPrepThreads) {
+        double xv = xsrc[i];
+        for (int j = 0; j < d; ++j) {
+            double v = src[(int64_t)j * N + i];
+            const double* row = S + j * LD;
+            for (int m = 0; m < j; ++m) v = fma(-row[m], stash[m * kPrepThreads], v);
+            v /= row[j];
+            stash[j * kPrepThreads] = v;
+            dst[(int64_t)j * N + i] = v;
+            xv = fma(-S[d * LD + j], v, xv);
+        }
+        xdst[i] = xv;
+    }
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p, int splits)
+{
+    extern __shared__ __align__(16) double sm[];
     __shared__ double red[32];
-    const int64_t b = blockIdx.x, N = p.N;
+    __shared__ int flag;
+    cg::cluster_group cluster = cg::this_cluster();
+    const int C = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
+    const int64_t b = blockIdx.y, N = p.N;
     const int d = p.d;
+    const PrepSmem L = prep_smem(d, splits);
     const double* t = p.t + b * N;
     const double* x = p.x + b * N;
     const double* w = p.w + b * N;
@@ -73,71 +247,76 @@ __global__ void __launch_bounds__(TH) prep_kernel(PrepParams p)
     double* psi = p.psi + b * (int64_t)d * N;  // [d][N]
     double* xt = p.xt + b * N;                 // [N]
     SeriesInfo* info = p.info + b;
+    const int64_t i0 = N * rank / C, i1 = N * (rank + 1) / C;  // this CTA's observations
+    double* scal = sm + L.scal;
 
     // ---- a1: validate, W = <1>, time origin --------------------------------------------
-    double bad = 0.0, neg = 0.0, wsum = 0.0, tmin = INFINITY, tmax = -INFINITY;
-    for (int64_t i = threadIdx.x; i < N; i += TH) {
-        double ti = t[i], xi = x[i], wi = w[i];
-        if (!isfinite(ti) || !isfinite(xi) || !isfinite(wi)) bad = 1.0;
-        if (wi < 0.0) neg = 1.0;
+    double bad = 0.0, wsum = 0.0, tmin = INFINITY, tmax = -INFINITY;
+    for (int64_t i = i0 + threadIdx.x; i < i1; i += kPrepThreads) {
+        const double ti = t[i], xi = x[i], wi = w[i];
+        if (!isfinite(ti) || !isfinite(xi) || !isfinite(wi) || wi < 0.0) bad = 1.0;
         wsum += wi;
         tmin = fmin(tmin, ti);
         tmax = fmax(tmax, ti);
         for (int j = 0; j < d; ++j)
             if (!isfinite(base[(int64_t)j * N + i])) bad = 1.0;
     }
-    bad = block_sum<TH>(bad + neg, red);
-    const double W = block_sum<TH>(wsum, red);
-    tmin = block_min<TH>(tmin, red);
-    tmax = -block_min<TH>(-tmax, red);
+    bad = block_sum(bad, red);
+    wsum = block_sum(wsum, red);
+    tmin = block_min(tmin, red);
+    tmax = -block_min(-tmax, red);
+    if (threadIdx.x == 0) {
+        scal[0] = bad;
+        scal[1] = wsum;
+        scal[2] = tmin;
+        scal[3] = tmax;
+    }
+    cluster.sync();
+    double W = 0.0;
+    bad = 0.0;
+    tmin = INFINITY;
+    tmax = -INFINITY;
+    for (int r = 0; r < C; ++r) {  // rank order: every CTA gets the same W
+        const double* rs = cluster.map_shared_rank(scal, r);
+        bad += rs[0];
+        W += rs[1];
+        tmin = fmin(tmin, rs[2]);
+        tmax = fmax(tmax, rs[3]);
+    }
     int status = 0;
     if (bad != 0.0 || !(W > 0.0) || !isfinite(W)) status = -2;  // FREDEC_EDATA
     const double t_mid = 0.5 * (tmin + tmax);
 
-    // ---- a2: orthonormal base psi (MGS, two sweeps) and residual x~ -----------------------
-    if (status == 0) {
-        for (int j = 0; j < d; ++j) {
-            double* v = psi + (int64_t)j * N;
-            for (int64_t i = threadIdx.x; i < N; i += TH) v[i] = base[(int64_t)j * N + i];
-            __syncthreads();
-            const double n0 = wdot<TH>(w, v, v, N, red);
-            for (int sweep = 0; sweep < 2; ++sweep)
-                for (int k = 0; k < j; ++k) {
-                    const double* q = psi + (int64_t)k * N;
-                    const double r = wdot<TH>(w, q, v, N, red);
-                    for (int64_t i = threadIdx.x; i < N; i += TH) v[i] = fma(-r, q[i], v[i]);
-                    __syncthreads();
-                }
-            const double n1 = wdot<TH>(w, v, v, N, red);
-            if (!(n1 > kTauBase * n0)) {
-                status = -3;  // FREDEC_ESINGULAR (uniform across the block)
-                break;
-            }
-            const double inv = 1.0 / sqrt(n1);
-            for (int64_t i = threadIdx.x; i < N; i += TH) v[i] *= inv;
-            __syncthreads();
-        }
+    // ---- a2: orthonormal base psi and residual x~ by two passes of Cholesky QR ----------------
+    // (with invalid data the passes run on whatever is there and the results are ignored: no CTA may
+    // leave the cluster's barriers)
+    for (int pass = 0; pass < 2; ++pass) {
+        const double* src = pass == 0 ? base : psi;
+        const double* xsrc = pass == 0 ? x : xt;
+        gram_partial(L, sm, w, src, xsrc, N, d, i0, i1);
+        gram_cluster_sum(L, sm, cluster);
+        // pass 0 decides whether the base functions are dependent (S6b); pass 1 factors a matrix
+        // that is the identity up to the first pass's orthogonality error
+        const bool ok = chol_with_x(L, sm, d, pass == 0 ? kTauBase : 0.0, &flag);
+        if (!ok && status == 0) status = -3;  // FREDEC_ESINGULAR (the same decision in every CTA)
+        if (ok) apply_factor(L, sm, d, src, xsrc, psi, xt, N, i0, i1);
     }
     double chi2 = 0.0;
-    if (status == 0) {
-        for (int64_t i = threadIdx.x; i < N; i += TH) xt[i] = x[i];
-        __syncthreads();
-        for (int sweep = 0; sweep < 2; ++sweep)
-            for (int k = 0; k < d; ++k) {
-                const double* q = psi + (int64_t)k * N;
-                const double r = wdot<TH>(w, q, xt, N, red);
-                for (int64_t i = threadIdx.x; i < N; i += TH) xt[i] = fma(-r, q[i], xt[i]);
-                __syncthreads();
-            }
-        chi2 = wdot<TH>(w, xt, xt, N, red);
-    }
-    if (threadIdx.x == 0) {
+    for (int64_t i = i0 + threadIdx.x; i < i1; i += kPrepThreads) chi2 = fma(w[i] * xt[i], xt[i], chi2);
+    chi2 = block_sum(chi2, red);
+    cluster.sync();  // the a1 scalars have been read by every CTA
+    if (threadIdx.x == 0) scal[0] = chi2;
+    cluster.sync();
+    if (rank == 0 && threadIdx.x == 0) {
+        double total = 0.0;
+        for (int r = 0; r < C; ++r) total += cluster.map_shared_rank(scal, r)[0];
         info->W = W;
-        info->chi2_base = chi2;
+        info->chi2_base = status == 0 ? total : 0.0;
         info->t_mid = t_mid;
         info->status = status;
         info->pad = 0;
     }
+    cluster.sync();  // no CTA exits while its shared memory may still be read
 }
 
 // ---- a3: per-observation table and seed records --------------------------
@@ -211,11 +390,35 @@ cudaError_t launch_table(const TableParams& p, int64_t B, cudaStream_t stream)
 
 cudaError_t launch_prep(const PrepParams& p, int64_t B, cudaStream_t stream)
 {
-    if (B >= 64 || p.N <= 2048)
-        prep_kernel<kPrepThreadsMin><<<(unsigned)B, kPrepThreadsMin, 0, stream>>>(p);
-    else
-        prep_kernel<kPrepThreadsMax><<<(unsigned)B, kPrepThreadsMax, 0, stream>>>(p);
-    return cudaGetLastError();
+    // CTAs per series: one per ~16k input values, at most 8 (a portable cluster), one when there are many series
+    int C = 1;
+    if (B <= 64)
+        while (C < kPrepMaxCluster && (int64_t)p.N * (p.d + 2) > (int64_t)16384 * C) C *= 2;
+    const int64_t slice = (p.N + C - 1) / C;
+    const PrepSmem probe = prep_smem(p.d, 1);
+    int splits = kPrepWarps / probe.tiles;
+    if (splits > (int)(slice / kGramMinSplit)) splits = (int)(slice / kGramMinSplit);
+    if (splits < 1) splits = 1;
+    const PrepSmem L = prep_smem(p.d, splits);
+    static size_t attr_smem = 0;
+    if (L.total > attr_smem) {
+        cudaError_t e = cudaFuncSetAttribute(prep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total);
+        if (e != cudaSuccess) return e;
+        attr_smem = L.total;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)C, (unsigned)B, 1);
+    cfg.blockDim = dim3(kPrepThreads, 1, 1);
+    cfg.dynamicSmemBytes = L.total;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)C;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, prep_kernel, p, splits);
 }
 
 }  // namespace fredec

@@ -1,28 +1,34 @@
-// refine_kernel.cuh -- local multifrequency fit (section 3, eq. 17): Gauss-Newton
-// over the frequencies with the linear coefficients re-fitted exactly at every iteration.
+// refine_kernel.cuh -- local multifrequency fits (section 3, eq. 17): Gauss-Newton
+// over the frequencies with the linear coefficients re-fitted exactly at every iteration, for a batch of
+// tuples drawn from one pool (phase 2 tabulates l_{m,loc} for the subsets of the pool;
+// "many entirely independent instances of the fitting subroutine").
 #pragma once
 #include "common.cuh"
 
 namespace fredec {
 
-// rows [3n+1][N] of the model functions at the current frequencies, times centred on t0:
-//   row 0 = 1, rows 2k+1 / 2k+2 = cos / sin(2 pi f_k t'), and, when theta != nullptr, rows 2n+1+k =
-//   d mu / d f_k = 2 pi t' (-a_k sin + b_k cos) with (a_k, b_k) = theta[2k+1], theta[2k+2]   (eq. 2's derivative)
-cudaError_t launch_model_rows(const double* t, int64_t N, double t0, const double* freqs, int n, const double* theta,
-                              double* rows, cudaStream_t stream);
+struct RefineParams {
+    const double* t;       // [N]
+    const double* x;       // [N]
+    const double* w;       // [N]
+    const double* bw;      // [4] output of launch_bandwidth: T_eff, Var t, weighted mean of t, status
+    const double* pool;    // [n_pool] starting frequencies
+    const int64_t* masks;  // [T] bit j selects pool[j]; nullptr: every tuple is the whole pool
+    double* freqs_out;     // [T][n_pool] refined frequencies (pool[j] where bit j is clear)
+    double* l_out;         // [T] min chi2 at the returned frequencies (0 on failure)
+    int32_t* iters_out;    // [T] frequency updates made
+    int32_t* status_out;   // [T] 0, -3 (singular normal equations) or -2 (bad t / w)
+    int64_t N;
+    int n_pool, max_iter;
+    double tol;
+};
 
-// Solves the normal equations held in the augmented Gram matrix A [(m+1)][(m+1)] (last row/column =
-// <x phi>, <x^2>) by Cholesky: theta [m] = Q^{-1} g, out2[0] = l = D - |L^{-1} g|^2,
-// out2[1] = status (0, or -3 when a pivot^2 <= 1e-12 x its diagonal).  One CTA.  m <= 76.
-cudaError_t launch_chol_solve(const double* A, int m, double* theta, double* out2, cudaStream_t stream);
-
-// Gauss-Newton step from the Gram matrix G [(m+1)][(m+1)] of (Phi [2n+1], dmu/df [n], x), m = 3n+1, and
-// the linear fit theta: g_f = <(x - mu) J> (its theta part vanishes), Q_f = <J J^T>,
-// step = Q_f^{-1} g_f; df_out [n] = its frequency part, clamped to +-max_step.  out2 as above.
-cudaError_t launch_gn_step(const double* G, int n, const double* theta, double max_step, double* df_out,
-                           double* out2, cudaStream_t stream);
-
-// freqs[k] += df[k]
-cudaError_t launch_axpy_small(double* freqs, const double* df, int n, cudaStream_t stream);
+// One CTA per tuple; m_max >= the largest number of selected frequencies of any tuple (sizes the shared
+// memory).  Model: constant + m sinusoids (eq. 2), times centred on their weighted mean.
+// Per iteration: Gram matrix of (1, cos, sin, t' cos, t' sin, x) in one sweep -> exact linear fit by
+// Cholesky (eq. 14) -> Q_f, g_f of eq. 17 from the same matrix -> step Q_f^{-1} g_f, its frequency part
+// clamped to +-0.5 / T_eff (reading R1) -> stop when max |step| T_eff <= tol (reading R2).
+cudaError_t launch_refine_batched(const RefineParams& p, int64_t T, int m_max, cudaStream_t stream);
+size_t refine_batched_smem(int m_max);
 
 }  // namespace fredec

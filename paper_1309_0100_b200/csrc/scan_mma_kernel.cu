@@ -68,8 +68,20 @@ namespace {
 constexpr int kNW = 8;         // MMA warps per CTA (two per SM sub-partition)
 constexpr int kSeedWarps = 4;  // seed warps per CTA (one per SM sub-partition)
 constexpr int kThreads = (kNW + kSeedWarps) * 32;
-// registers per thread after setmaxnreg: 128 * (2 * kRegsMma + kRegsSeed) <= 65536
-constexpr int kRegsMma = 216, kRegsSeed = 72;
+// Registers per thread after setmaxnreg.  The CTA is launched with kLaunchRegs registers for each of its
+// 384 threads, and that pool is all setmaxnreg can redistribute (an increase beyond it waits for ever):
+// 8 mma + 4 seed <= 12 kLaunchRegs.  The accumulators of an MMA thread are 2 * NOCT * (NB + 2) * H
+// registers; up to 176 of them leave 72 registers to the seed warps, 192 (the largest tiles: the fewest
+// seeds per MMA) leave 40.
+constexpr int kLaunchRegs = 168;  // 65536 / 384 rounded down to the allocation unit of 8
+template <int H, int NOCT, int NB>
+struct ScanRegs {
+    static constexpr int kAcc = 2 * NOCT * (NB + 2) * H;
+    static constexpr int kMma = kAcc > 176 ? 232 : 216;
+    static constexpr int kSeed = kAcc > 176 ? 40 : 72;
+    static_assert(kAcc <= 192, "accumulators do not fit the MMA warps' registers");
+    static_assert(kNW * kMma + kSeedWarps * kSeed <= (kNW + kSeedWarps) * kLaunchRegs, "register pool exceeded");
+};
 
 constexpr int kSeedGroups = 2;  // groups of 4 observations per seed warp and step at most (TI <= 32): one per half warp
 
@@ -249,6 +261,14 @@ struct RingPos {
     bool ready;
 };
 
+// 2 x for a finite |x| < 2^1023 by an exponent increment on the integer pipe.  x = +-0 gives +-2^-1022
+// (an absolute error of 2e-308) and a subnormal x a value below 2^-1021: both far below one rounding
+// error of the sums they enter.
+__device__ __forceinline__ double twice(double x)
+{
+    return __hiloint2double(__double2hiint(x) + 0x00100000, __double2loint(x));
+}
+
 // a6 for one group of 4 observations: A fragments (seeds), B fragments (table), 2 * NF * NT MMAs per unit.
 template <int CNT, int H, int NOCT, int NB>
 __device__ __forceinline__ void mma_group(Tiles<H, NOCT, NB>& acc, const double2* tk, const double2* sk)
@@ -259,8 +279,11 @@ __device__ __forceinline__ void mma_group(Tiles<H, NOCT, NB>& acc, const double2
 #pragma unroll
     for (int o = 0; o < CNT; ++o) {
         a[o] = sk[o * 32];
-        c2[o] = fma(a[o].x, a[o].x, -(a[o].y * a[o].y));  // cos 2 phi
-        s2[o] = (a[o].x + a[o].x) * a[o].y;              // sin 2 phi
+        // double-angle seeds with two FP64 instructions (every scalar FP64 instruction of an MMA warp
+        // takes pipe cycles from the MMAs): 2 cos phi comes from the integer unit
+        const double tc = twice(a[o].x);
+        c2[o] = fma(tc, a[o].x, -1.0);  // cos 2 phi = 2 cos^2 phi - 1
+        s2[o] = tc * a[o].y;            // sin 2 phi = 2 cos phi sin phi
     }
 #pragma unroll
     for (int f = 0; f < NF; ++f) {
@@ -283,6 +306,145 @@ __device__ __forceinline__ void mma_group(Tiles<H, NOCT, NB>& acc, const double2
                 }
             }
         }
+    }
+}
+
+// ---- a6 with an explicit instruction order, for the configurations whose accumulators take 192 registers.
+// With 40 registers left, the compiler's own schedule of mma_group (table loads hoisted far ahead)
+// runs out of registers and pays for it in register moves, each of which costs the MMA stream an issue
+// cycle.  Here the order is fixed with volatile asm: the 16-byte table loads run kDepth - 1 loads (8 or
+// 12 MMAs) ahead of their MMAs and continue into the next group; the w family comes last in a group, its
+// double-angle seeds are formed as one pair of adjacent FP64 instructions (a pair costs the MMA stream
+// about as much as one single instruction) and the next group's seeds are loaded once the current ones
+// are dead.
+#define FREDEC_DMMA_V(c, a, b)                                                                       \
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"     \
+                 : "+d"((c)[0]), "+d"((c)[1])                                                        \
+                 : "d"(a), "d"(b))
+
+__device__ __forceinline__ double2 lds128(uint32_t addr)
+{
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+
+// State of the load pipeline of one warp inside a ring slot.
+template <int D>
+struct LoadPipe {
+    double2 a;     // seeds of the current group
+    double2 b[D];  // table loads in flight
+};
+
+// One group of 4 observations of one unit (NOCT = 1).  tk / sk: shared-memory addresses of this lane's
+// table fragments / seeds of the group; tk_next / sk_next: those of the group that follows (== tk / sk
+// after the last one: the values are then loaded again and not used).
+template <int H, int NB, int D>
+__device__ __forceinline__ void mma_group_pipelined(Tiles<H, 1, NB>& acc, LoadPipe<D>& lp, uint32_t tk, uint32_t sk,
+                                                    uint32_t tk_next, uint32_t sk_next)
+{
+    constexpr int NT = H / 4, NF = NB + 2, NP = NF * NT / 2, PW = (NF - 1) * (NT / 2);  // PW: first load of the w family
+    static_assert(NP % D == 0 && PW >= 2, "load ring must divide the loads of a group");
+    double c2 = 0.0, s2 = 0.0;
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        const int q = p + D - 1;  // the load issued now
+        lp.b[q % D] = q < NP ? lds128(tk + q * 512) : lds128(tk_next + (q - NP) * 512);
+        if (p == PW - 1) {
+            const double tc = twice(lp.a.x);
+            asm volatile("fma.rn.f64 %0, %2, %3, 0dBFF0000000000000;\n\tmul.rn.f64 %1, %2, %4;"
+                         : "=&d"(c2), "=&d"(s2)
+                         : "d"(tc), "d"(lp.a.x), "d"(lp.a.y));  // cos 2 phi = 2 cos^2 phi - 1, sin 2 phi = 2 cos phi sin phi
+        }
+        const int f = p / (NT / 2), t0 = 2 * (p % (NT / 2));
+        const double2 bb = lp.b[p % D];
+        if (f < NF - 1) {
+            FREDEC_DMMA_V(acc.v[0][0][f][t0], lp.a.x, bb.x);
+            FREDEC_DMMA_V(acc.v[0][1][f][t0], lp.a.y, bb.x);
+            FREDEC_DMMA_V(acc.v[0][0][f][t0 + 1], lp.a.x, bb.y);
+            FREDEC_DMMA_V(acc.v[0][1][f][t0 + 1], lp.a.y, bb.y);
+        } else {
+            if (p == PW) lp.a = lds128(sk_next);  // the current seeds are dead from here on
+            FREDEC_DMMA_V(acc.v[0][0][f][t0], c2, bb.x);
+            FREDEC_DMMA_V(acc.v[0][1][f][t0], s2, bb.x);
+            FREDEC_DMMA_V(acc.v[0][0][f][t0 + 1], c2, bb.y);
+            FREDEC_DMMA_V(acc.v[0][1][f][t0 + 1], s2, bb.y);
+        }
+    }
+}
+
+// The loads of a group's successor are issued whether or not there is one (no selects in the loop): past
+// the last group of a slot they read the slot's own seed area, the next slot, or the kPipePad bytes the
+// launch adds behind the ring, and the values are not used.
+constexpr int kPipePad = 8192;
+
+template <int H, int NB>
+__device__ __forceinline__ void round_mma_pipelined(Tiles<H, 1, NB>& acc, RingPos& rp, const unsigned char* smem,
+                                                    size_t slot_bytes, size_t tab_bytes, int NS, int KS, int64_t G4,
+                                                    int tile0, int tile1, WarpRole role, int lane, uint64_t* bar_tab,
+                                                    uint64_t* bar_seed, uint64_t* bar_done)
+{
+    constexpr int NT = H / 4, NF = NB + 2, CAP = kNW, D = 3;
+    constexpr uint32_t GROUP_B = NF * NT * 32 * 8, SEED_B = CAP * 32 * 16;  // bytes per group: table, seeds
+    static_assert(SEED_B + 16 <= kPipePad && (D - 1) * 512 <= kPipePad, "padding behind the ring too small");
+    const int64_t g_end = min((int64_t)tile1 * KS, G4);
+#pragma unroll 1
+    for (int64_t g = (int64_t)tile0 * KS; g < g_end; g += KS) {
+        const int ngrp = (int)min((int64_t)KS, g_end - g);
+        if (!rp.ready) {
+            mbar_wait(&bar_tab[rp.slot], rp.par);
+            mbar_wait(&bar_seed[rp.slot], rp.par);
+        }
+        const uint32_t base = smem_u32(smem + rp.slot * slot_bytes);
+        int nslot = rp.slot + 1;
+        uint32_t npar = rp.par;
+        if (nslot == NS) {
+            nslot = 0;
+            npar ^= 1u;
+        }
+        uint32_t tk = base + lane * 16;
+        uint32_t sk = base + (uint32_t)tab_bytes + (role.off * 32 + lane) * 16;
+        rp.ready = false;
+        LoadPipe<D> lp;
+        if (role.S == 1) {
+            // every group of the slot, two per iteration; the next slot's barriers are looked at two or
+            // three groups before the end, so that the MMA stream continues across slots
+            lp.a = lds128(sk);
+#pragma unroll
+            for (int q = 0; q < D - 1; ++q) lp.b[q] = lds128(tk + q * 512);
+            int left = ngrp;
+#pragma unroll 1
+            for (; left >= 2; left -= 2) {
+                if (left <= 3) rp.ready = mbar_test(&bar_tab[nslot], npar) & mbar_test(&bar_seed[nslot], npar);
+                mma_group_pipelined<H, NB, D>(acc, lp, tk, sk, tk + GROUP_B, sk + SEED_B);
+                mma_group_pipelined<H, NB, D>(acc, lp, tk + GROUP_B, sk + SEED_B, tk + 2 * GROUP_B, sk + 2 * SEED_B);
+                tk += 2 * GROUP_B;
+                sk += 2 * SEED_B;
+            }
+            if (left == 1) {
+                if (ngrp == 1) rp.ready = mbar_test(&bar_tab[nslot], npar) & mbar_test(&bar_seed[nslot], npar);
+                mma_group_pipelined<H, NB, D>(acc, lp, tk, sk, tk + GROUP_B, sk + SEED_B);
+            }
+        } else if (role.sp < ngrp) {
+            // a8: the S warps of a unit take the slot's groups in turn
+            const uint32_t tstep = GROUP_B * role.S, sstep = SEED_B * role.S;
+            tk += role.sp * GROUP_B;
+            sk += role.sp * SEED_B;
+            lp.a = lds128(sk);
+#pragma unroll
+            for (int q = 0; q < D - 1; ++q) lp.b[q] = lds128(tk + q * 512);
+#pragma unroll 1
+            for (int ks = role.sp; ks < ngrp; ks += role.S) {
+                const bool last = ks + role.S >= ngrp;
+                mma_group_pipelined<H, NB, D>(acc, lp, tk, sk, last ? tk : tk + tstep, last ? sk : sk + sstep);
+                tk += tstep;
+                sk += sstep;
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bar_done[rp.slot]);
+        rp.slot = nslot;
+        rp.par = npar;
     }
 }
 
@@ -496,7 +658,7 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
 
     if (wid >= kNW) {
         // ================= seed warps: table staging (a4) + seeds (a5) =====================
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegsSeed));
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(ScanRegs<H, NOCT, NB>::kSeed));
         const int pw = wid - kNW;
         // lane = (j, mp, k): group pw + 4 j of the slot, observation k of it, runs mp and mp + 4 of each
         // unit.  One exact evaluation per lane and step serves two runs (the second by a rotation).
@@ -567,7 +729,7 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
         }
     } else {
         // ================= MMA warps: a6 (as a contraction), a9, a10 ========================
-        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegsMma));
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(ScanRegs<H, NOCT, NB>::kMma));
         Tiles<H, NOCT, NB> acc;
         acc.clear();
         RingPos rp = {0, 0u, false};
@@ -576,7 +738,10 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
 #define FREDEC_ROUND(CNT) \
     round_mma<CNT>(acc, rp, smem_raw, slot_bytes, tab_bytes, NS, KS, p.G4, c.tile, c.tile_end, role, lane, bar_tab, \
                    bar_seed, bar_done)
-            if (NOCT == 1 || role.cnt == 1) {
+            if constexpr (ScanRegs<H, NOCT, NB>::kAcc > 176) {
+                round_mma_pipelined<H, NB>(acc, rp, smem_raw, slot_bytes, tab_bytes, NS, KS, p.G4, c.tile, c.tile_end,
+                                           role, lane, bar_tab, bar_seed, bar_done);
+            } else if (NOCT == 1 || role.cnt == 1) {
                 FREDEC_ROUND(1);
             } else if (NOCT == 2 || role.cnt == 2) {
                 FREDEC_ROUND((NOCT >= 2 ? 2 : 1));
@@ -689,7 +854,7 @@ __global__ void __launch_bounds__(kNW * 32) tail_solve_kernel(MmaScanParams p)
 template <int H, int NOCT, int NB>
 cudaError_t launch_one(const MmaScanParams& p, cudaStream_t stream)
 {
-    const size_t smem = (size_t)p.NS * mma_scan_slot_bytes(NB, p.TI);
+    const size_t smem = (size_t)p.NS * mma_scan_slot_bytes(NB, p.TI) + kPipePad;
     static size_t attr_smem = 0;
     if (smem > attr_smem) {
         cudaError_t e = cudaFuncSetAttribute(scan_mma_kernel<H, NOCT, NB>,
@@ -707,9 +872,11 @@ cudaError_t launch_one(const MmaScanParams& p, cudaStream_t stream)
 
 }  // namespace
 
-// (H, NOCT) per NB: NOCT * (2 + NB) * H accumulator doubles per thread
+// (H, NOCT) per NB: NOCT * (2 + NB) * H accumulator doubles per thread.  The seeds (the only FP64 scalar
+// work per pair) are one complex number per (run of 2H frequencies, observation): the longest run the
+// registers allow, 96 accumulator doubles, for d <= 2 and d = 4.
 #define FREDEC_MMA_CONFIGS(X) \
-    X(16, 2, 0) X(16, 1, 1) X(16, 1, 2) X(8, 2, 3) X(8, 1, 4) X(8, 1, 5) X(8, 1, 6) X(8, 1, 7) X(8, 1, 8) X(8, 1, 9)
+    X(48, 1, 0) X(32, 1, 1) X(24, 1, 2) X(16, 1, 3) X(16, 1, 4) X(8, 1, 5) X(8, 1, 6) X(8, 1, 7) X(8, 1, 8) X(8, 1, 9)
 
 MmaScanConfig mma_scan_config(int NB)
 {

@@ -97,10 +97,12 @@ __global__ void __launch_bounds__(kStatThreads) sin_base_kernel(const double* __
 }
 
 __global__ void peak_stats_kernel(const double* __restrict__ dchi2, const int64_t* __restrict__ idx, int k,
-                                  double chi2_base, double NH, double W, double A1, double* __restrict__ out)
+                                  const SeriesInfo* __restrict__ info, double NH, double W, double A1,
+                                  double* __restrict__ out)
 {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= k) return;
+    const double chi2_base = info->status == 0 ? info->chi2_base : 0.0;
     const int64_t i = idx[j];
     const double z = i >= 0 ? zstat_of(dchi2[i], chi2_base, NH) : 0.0;
     out[2 * j] = z;
@@ -159,10 +161,10 @@ cudaError_t launch_sin_base(const double* t, int64_t N, const double* freqs, int
     return cudaGetLastError();
 }
 
-cudaError_t launch_peak_stats(const double* dchi2, const int64_t* idx, int k, double chi2_base, double NH, double W,
-                              double A1, double* out2k, cudaStream_t stream)
+cudaError_t launch_peak_stats(const double* dchi2, const int64_t* idx, int k, const SeriesInfo* info, double NH,
+                              double W, double A1, double* out2k, cudaStream_t stream)
 {
-    peak_stats_kernel<<<(k + 127) / 128, 128, 0, stream>>>(dchi2, idx, k, chi2_base, NH, W, A1, out2k);
+    peak_stats_kernel<<<(k + 127) / 128, 128, 0, stream>>>(dchi2, idx, k, info, NH, W, A1, out2k);
     return cudaGetLastError();
 }
 

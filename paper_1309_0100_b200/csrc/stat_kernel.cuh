@@ -24,8 +24,10 @@ cudaError_t launch_bandwidth(const double* t, const double* w, int64_t N, double
 cudaError_t launch_sin_base(const double* t, int64_t N, const double* freqs, int m, double* base_out,
                             cudaStream_t stream);
 
-// For the k peak indices idx[j] (-1 = unused): out[j] = (z, fap) of dchi2[idx[j]], as in zstat / fap1.
-cudaError_t launch_peak_stats(const double* dchi2, const int64_t* idx, int k, double chi2_base, double NH, double W,
-                              double A1, double* out2k, cudaStream_t stream);
+// For the k peak indices idx[j] (-1 = unused): out[j] = (z, fap) of dchi2[idx[j]], as in zstat / fap1, with
+// chi2_base read from the scan's per-series record in device memory (so that no host round trip separates
+// the scan from its peak statistics).
+cudaError_t launch_peak_stats(const double* dchi2, const int64_t* idx, int k, const SeriesInfo* info, double NH,
+                              double W, double A1, double* out2k, cudaStream_t stream);
 
 }  // namespace fredec

@@ -4,10 +4,11 @@
 // -infinity.  Peaks are ranked by the TOTAL order (z descending, index ascending), so the
 // top-k set and its order are unique and the result is bit-exact whatever the traversal order.
 //
-// Each warp streams its share of z once (coalesced; the +-1 neighbours come from L1) and keeps
+// Each warp streams a contiguous segment of z once (16-byte loads, several in flight) and keeps
 // a sorted top-k list spread over its lanes' registers (rank r lives in slot r/32 of lane
-// r%32).  A candidate is first compared with the list's k-th entry, so almost all peaks cost
-// one comparison; the rare survivors are inserted with warp shuffles.  Warp lists are merged
+// r%32).  A whole step of 64 points is first compared with the list's k-th entry, so almost all
+// points cost a comparison and a share of one vote; the rare survivors are tested for being peaks
+// and inserted with warp shuffles.  Warp lists are merged
 // per CTA through shared memory, CTA lists by a second small kernel.  No atomics.
 #include <cmath>
 #include <cstdint>
@@ -19,9 +20,6 @@ namespace {
 
 #ifndef FREDEC_TOPK_THREADS
 #define FREDEC_TOPK_THREADS 256
-#endif
-#ifndef FREDEC_TOPK_UN
-#define FREDEC_TOPK_UN 4
 #endif
 constexpr int kTopkThreads = FREDEC_TOPK_THREADS;
 constexpr int kTopkWarps = kTopkThreads / 32;
@@ -152,6 +150,14 @@ __device__ void cta_merge_and_write(WarpList<SLOTS>& L, const TopkParams& p, int
     }
 }
 
+// 16-byte load of the two grid points [i, i + 1] of a row of K points (i even, the row 16-byte aligned);
+// points at or beyond K read as -infinity.
+__device__ __forceinline__ double2 load_pair(const double* __restrict__ z, int64_t i, int64_t K)
+{
+    if (i + 1 < K) return *reinterpret_cast<const double2*>(z + i);
+    return make_double2(i < K ? z[i] : -INFINITY, -INFINITY);
+}
+
 template <int SLOTS>
 __global__ void __launch_bounds__(kTopkThreads) topk_scan_kernel(TopkParams p)
 {
@@ -161,52 +167,55 @@ __global__ void __launch_bounds__(kTopkThreads) topk_scan_kernel(TopkParams p)
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int64_t b = blockIdx.y, K = p.K;
     const double* z = p.z + b * K;
-    // contiguous chunk of this CTA, a multiple of what the CTA covers per step
-    constexpr int UN = FREDEC_TOPK_UN;                               // 16-byte loads in flight per thread
-    constexpr int64_t kStep = kTopkThreads * 2;         // elements per CTA and sub-step
+    // contiguous chunk of this CTA, cut into one contiguous segment per warp (multiples of 64 points)
+    constexpr int64_t kStep = 64;  // points per warp and step: one 16-byte load per lane
     int64_t chunk = (K + p.nblk - 1) / p.nblk;
-    chunk = (chunk + kStep - 1) / kStep * kStep;
+    chunk = (chunk + kStep * kTopkWarps - 1) / (kStep * kTopkWarps) * (kStep * kTopkWarps);
     const int64_t begin = (int64_t)blockIdx.x * chunk;
     const int64_t end = min(K, begin + chunk);
+    const int64_t seg = chunk / kTopkWarps;
+    const int64_t s0 = begin + wid * seg, s1 = min(end, s0 + seg);
 
     WarpList<SLOTS> L;
     L.init(p.k, lane);
     if ((reinterpret_cast<uintptr_t>(z) & 15) == 0) {
-        // each lane owns two adjacent elements per sub-step (one 16-byte load); their outer
-        // neighbours come from the adjacent lanes, the warp's two outer neighbours from L1/L2
-        for (int64_t base = begin + wid * 64; base < end; base += kStep * UN) {
-            double2 v[UN];
-            double lft[UN], rgt[UN];
+        // The warp walks its segment in steps of 64 points, kRing - 1 loads ahead.  A step is looked at
+        // closely only if some lane's point could enter the list (z >= the list's k-th entry; until k peaks
+        // are known that entry is -infinity and every step is): almost every step costs one load, two
+        // comparisons and a vote.  The neighbours of a lane's two points are its own, the adjacent
+        // lanes' (shuffles) and, at the warp's edges, the previous / next step's.
+        constexpr int kRing = 4;
+        double2 ring[kRing];
 #pragma unroll
-            for (int u = 0; u < UN; ++u) {
-                const int64_t i0 = base + u * kStep + 2 * lane;
-                v[u] = make_double2(-INFINITY, -INFINITY);
-                if (i0 + 1 < K) {
-                    v[u] = *reinterpret_cast<const double2*>(z + i0);
-                } else if (i0 < K) {
-                    v[u].x = z[i0];
+        for (int u = 0; u < kRing - 1; ++u) ring[u] = load_pair(z, s0 + u * kStep + 2 * lane, K);
+        double prev_c = s0 > 0 && s0 < K ? z[s0 - 1] : -INFINITY;  // the point before the step (lane 31's view)
+        for (int64_t base = s0; base < s1; base += kStep * kRing) {
+#pragma unroll
+            for (int u = 0; u < kRing; ++u) {
+                const int64_t sb = base + u * kStep;  // this step
+                if (sb >= s1) break;                  // warp-uniform
+                ring[(u + kRing - 1) % kRing] = load_pair(z, sb + (kRing - 1) * kStep + 2 * lane, K);
+                const double2 cur = ring[u], nxt = ring[(u + 1) % kRing];
+                if (__any_sync(0xffffffffu, cur.x >= L.thr_z || cur.y >= L.thr_z)) {
+                    const int64_t i0 = sb + 2 * lane;
+                    const double a = sanitize(cur.x), c = sanitize(cur.y);
+                    const double up = __shfl_up_sync(0xffffffffu, c, 1), dn = __shfl_down_sync(0xffffffffu, a, 1);
+                    const double first_next = sanitize(__shfl_sync(0xffffffffu, nxt.x, 0));
+                    const double last_prev = sanitize(__shfl_sync(0xffffffffu, prev_c, 31));
+                    const double l = lane == 0 ? last_prev : up;
+                    const double r = lane == 31 ? first_next : dn;
+                    L.offer(a, i0, i0 < s1 && a > l && a >= c);
+                    L.offer(c, i0 + 1, i0 + 1 < s1 && c > a && c >= r);
                 }
-                lft[u] = (lane == 0 && i0 > 0 && i0 < K) ? z[i0 - 1] : -INFINITY;
-                rgt[u] = (lane == 31 && i0 + 2 < K) ? z[i0 + 2] : -INFINITY;
-            }
-#pragma unroll
-            for (int u = 0; u < UN; ++u) {
-                const int64_t i0 = base + u * kStep + 2 * lane;
-                if (base + u * kStep >= end) break;  // warp-uniform
-                const double a = sanitize(v[u].x), c = sanitize(v[u].y);
-                const double up = __shfl_up_sync(0xffffffffu, c, 1), dn = __shfl_down_sync(0xffffffffu, a, 1);
-                const double l = lane == 0 ? sanitize(lft[u]) : up;
-                const double r = lane == 31 ? sanitize(rgt[u]) : dn;
-                L.offer(a, i0, i0 < K && a > l && a >= c);
-                L.offer(c, i0 + 1, i0 + 1 < K && c > a && c >= r);
+                prev_c = cur.y;
             }
         }
     } else {
-        for (int64_t base = begin + wid * 32; base < end; base += kTopkThreads) {
-            const int64_t i = base + lane;
+        for (int64_t base = s0 + lane; base - lane < s1; base += 32) {
+            const int64_t i = base;
             bool peak = false;
             double v = -INFINITY;
-            if (i < K) {
+            if (i < s1) {
                 v = sanitize(z[i]);
                 const double l = i > 0 ? sanitize(z[i - 1]) : -INFINITY;
                 const double r = i + 1 < K ? sanitize(z[i + 1]) : -INFINITY;

@@ -20,9 +20,15 @@ def fr():
 
 
 def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "fredec.h")).read()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(fredec_[a-z0-9_]+)\s*\(", text)))
+    """Every function any header under include/ declares (fredec.h: the product ABI; fredec_bench.h: the
+    measurement probes)."""
+    names = set()
+    inc = os.path.join(ROOT, "include")
+    for h in sorted(os.listdir(inc)):
+        if h.endswith(".h"):
+            text = re.sub(r"/\*.*?\*/", "", open(os.path.join(inc, h)).read(), flags=re.S)
+            names |= set(re.findall(r"\b(fredec_[a-z0-9_]+)\s*\(", text))
+    return sorted(names)
 
 
 def test_header_symbols_are_exported_and_bound(fr):

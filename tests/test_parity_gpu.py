@@ -35,6 +35,12 @@ def gpu_scan(fr, t, x, w, base, f0, df, K, device=True):
     return fr.fredec_scan(t, x, w, base, f0, df, K)
 
 
+def run_length(d):
+    """Frequencies per run of the scan kernel's configuration for d base functions (DESIGN.md section 5;
+    for d > 9 the passes use 8 functions each)."""
+    return {0: 96, 1: 64, 2: 48, 3: 32, 4: 32}.get(d, 16)
+
+
 def assert_parity(z_gpu, z_ref, what=""):
     zmax = float(np.max(z_ref))
     err = float(np.max(np.abs(z_gpu - z_ref)))
@@ -161,12 +167,12 @@ def test_ragged_sizes(fr, oracle_mod, N, K):
     assert_parity(z, z_ref, f"N={N},K={K}")
 
 
-@pytest.mark.parametrize("d,units", [(2, 1), (2, 2), (2, 3), (2, 4), (2, 7), (2, 13), (1, 5), (0, 6), (3, 11), (9, 3), (9, 9)])
+@pytest.mark.parametrize("d,units", [(2, 1), (2, 2), (2, 3), (2, 4), (2, 7), (2, 13), (1, 5), (0, 6), (3, 11), (4, 5), (4, 2), (9, 3), (9, 9)])
 def test_round_compositions_and_observation_split(fr, oracle_mod, d, units):
     """Row a8: a grid of `units` 8-run MMA tiles is processed in rounds of 8, 4, 2 and 1 tiles; rounds of
     fewer than 8 split the observations 2, 4 or 8 ways between warps and add the partial sums.  K is
     chosen so that the last tile is ragged as well; N spans several ring slots and a ragged last one."""
-    run = 32 if d <= 2 else 16                 # frequencies per run (DESIGN.md section 5)
+    run = run_length(d)
     K = units * 8 * run - 5
     t, x, w, base = inputs.random_series(9000 + 17 * d + units, 203, d)
     f0, df = 0.003, 0.37 / K
@@ -236,6 +242,74 @@ def test_host_and_device_pointers_agree_bitwise(fr):
     zb = gpu_scan(fr, t, x, w, base, wl.f0, wl.df, wl.K, device=False)
     zc = gpu_scan(fr, t, x, w, base, wl.f0, wl.df, wl.K, device=True)
     assert np.array_equal(za, zb) and np.array_equal(za, zc)      # also: run-to-run reproducible
+
+
+@pytest.mark.parametrize("N,d", [(600, 9), (2000, 51), (5000, 2), (20_000, 33), (3000, 64), (70, 64)])
+def test_prep_cluster_sizes_and_base_fit(fr, oracle_mod, N, d):
+    """Rows a1/a2 (base orthogonalisation by two passes of Cholesky QR, one thread-block cluster per
+    series): sizes that run on 1, 2, 4 and 8 CTAs per series, up to FREDEC_D_MAX functions.  chi2_base
+    against the oracle's Cholesky of the raw functions to 1e-12, and a short scan against the oracle
+    (the scan's Schur complement is exact only if psi is orthonormal and x~ orthogonal to it)."""
+    t, x, w, base = inputs.random_series(5000 + N + d, N, d, t_span=400.0)
+    chi2 = fr.fredec_chi2_base(t, x, w, base)
+    chi2_ref = oracle_mod.chi2_base(t, x, w, base)
+    assert abs(chi2 - chi2_ref) <= 1e-12 * chi2_ref
+    f0, df, K = 0.013, 0.0021, 301
+    z_ref = oracle_mod.scan(t, x, w, base, f0, df, K, threads=0)
+    z = gpu_scan(fr, t, x, w, base, f0, df, K)
+    assert_parity(z, z_ref, f"N={N},d={d}")
+    assert np.array_equal(z, gpu_scan(fr, t, x, w, base, f0, df, K))
+
+
+def test_prep_dependent_base_is_singular(fr):
+    """DESIGN.md S6b: a base function in the span of the others is FREDEC_ESINGULAR, wherever it stands."""
+    import paper_1309_0100_b200 as m
+    t, x, w, base = inputs.random_series(11, 300, 6)
+    for pos in (1, 3, 5):
+        dep = base.copy()
+        dep[pos] = 2.0 * base[0] - 0.5 * base[(pos + 1) % 6 or 2]
+        with pytest.raises(m.FredecError) as e:
+            fr.fredec_scan(t, x, w, dep, 0.01, 0.01, 10)
+        assert e.value.code == m.FREDEC_ESINGULAR
+    nearly = base.copy()
+    nearly[4] = base[2] + 1e-4 * base[4]          # relative residual norm 1e-4 >> 1e-6: accepted
+    assert np.all(np.isfinite(fr.fredec_scan(t, x, w, nearly, 0.01, 0.01, 10)))
+
+
+def test_asynchronous_form(fr, oracle_mod):
+    """fredec_set_async (include/fredec.h): with device pointers the call returns once enqueued; after the
+    caller's synchronisation the outputs equal the synchronous call's bit for bit and fredec_last_status
+    gives the count / the data error.  Host pointers stay synchronous."""
+    import torch
+    wl = inputs.config(2, K=20_000)
+    t, x, w, base = wl.series(0)
+    dt, dx, dw, db = _dev(t, x, w, base)
+    z_sync, idx_sync, cnt_sync = fr.fredec_scan_topk(dt, dx, dw, db, wl.f0, wl.df, wl.K, 10)
+    fr.fredec_set_async(True)
+    try:
+        z = torch.empty(wl.K, dtype=torch.float64, device="cuda")
+        idx = torch.empty(10, dtype=torch.int64, device="cuda")
+        _, _, rc = fr.fredec_scan_topk(dt, dx, dw, db, wl.f0, wl.df, wl.K, 10, z_out=z, idx_out=idx)
+        assert rc == 0                                     # enqueued: the count comes from last_status
+        assert fr.fredec_last_status() == cnt_sync
+        torch.cuda.synchronize()
+        assert torch.equal(z, z_sync) and torch.equal(idx, idx_sync)
+        # two calls back to back without a host synchronisation in between
+        z2 = fr.fredec_scan(dt, dx, dw, db, wl.f0, wl.df, wl.K)
+        idx2, _ = fr.fredec_topk(z2, 10)
+        assert fr.fredec_last_status() == cnt_sync and torch.equal(idx2, idx_sync)
+        # a data error surfaces in last_status
+        bad = dx.clone(); bad[7] = float("nan")
+        fr.fredec_scan(dt, bad, dw, db, wl.f0, wl.df, wl.K)
+        with pytest.raises(fr.FredecError) as e:
+            fr.fredec_last_status()
+        assert e.value.code == fr.FREDEC_EDATA
+        # host pointers: synchronous as ever
+        zh, idxh, cnth = fr.fredec_scan_topk(t, x, w, base, wl.f0, wl.df, wl.K, 10)
+        assert cnth == cnt_sync and np.array_equal(zh, z_sync.cpu().numpy())
+    finally:
+        fr.fredec_set_async(False)
+    assert fr.fredec_scan_topk(dt, dx, dw, db, wl.f0, wl.df, wl.K, 10)[2] == cnt_sync
 
 
 def test_large_phase_accuracy(fr, oracle_mod):
@@ -404,7 +478,7 @@ def test_long_series_many_ring_laps(fr, oracle_mod):
     assert abs((f0 + df * int(np.argmax(z))) - 0.0371) < 2 * df
 
 
-@pytest.mark.parametrize("d,N", [(2, 150), (0, 90), (3, 131), (9, 70), (1, 33)])
+@pytest.mark.parametrize("d,N", [(2, 150), (0, 90), (3, 131), (4, 77), (9, 70), (1, 33)])
 def test_shared_tail_mode(fr, oracle_mod, d, N):
     """One series with at least one full round per SM: every CTA runs its full rounds, the left-over
     rounds are cut across the observations into segments whose partial sums the tail-solve kernel
@@ -412,8 +486,8 @@ def test_shared_tail_mode(fr, oracle_mod, d, N):
     which is only partly filled; few tiles per round, so that segments start and end inside rounds."""
     import torch
     sms = torch.cuda.get_device_properties(0).multi_processor_count
-    run = 32 if d <= 2 else 16                       # frequencies per run (DESIGN.md section 5)
-    cap = 16 if d in (0, 3) else 8                   # units per round
+    run = run_length(d)
+    cap = 8                                          # units per round
     units = sms * cap + 5 * cap + 3
     K = units * 8 * run - 7
     t, x, w, base = inputs.random_series(7000 + d, N, d, t_span=60.0)

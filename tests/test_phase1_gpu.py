@@ -211,7 +211,12 @@ def test_subset_fits_aliased_pools(fr, p1, which):
     incrementally updated L^{-1} loses digits.  Pools: (a) the pool the ORACLE's phase 1 finds on the
     config-2 series (seasonal gaps: yearly alias families); (b) the 0.6 ... 1.4 Hz comb of the alias
     example; (c) constructed near-duplicates 0.1/T, 1e-3/T and exactly 0 apart.
-    Tolerance as for the benign pools: 1e-10 D, D = <x^2>."""
+    Tolerance as for the benign pools, 1e-10 D (D = <x^2>), wherever the fit is conditioned well enough
+    for the oracle itself to be that accurate (smallest relative pivot >= 1e-4; measured against 40-digit
+    arithmetic the FP64 oracle is off by up to 1.7e-5 D on the full comb, whose Q has condition 3e16).
+    Below that both sides lose eps / pivot of D: bound 1e3 eps D / pivot down to pivot 1e-8; inside the
+    S6 band only validity (finite, 0 <= l <= l of the constant alone).  The worst cases per class are
+    written to gpurun_out/subset_alias_*.txt."""
     rng = np.random.Generator(np.random.PCG64(7))
     if which == "rv_like_pool":
         wl = inputs.config(2)
@@ -231,15 +236,23 @@ def test_subset_fits_aliased_pools(fr, p1, which):
     got = fr.fredec_subset_fits(t, x, w, freqs)
     masks = np.arange(1 << n) if n <= 10 else np.unique(np.concatenate(
         [[0, (1 << n) - 1], 1 << np.arange(n), rng.integers(0, 1 << n, 600)]))
-    ref = p1.subset_fits(t, x, w, freqs, masks=masks)
+    ref, pmin = p1.subset_fits(t, x, w, freqs, masks=masks, return_pivots=True)
     D = float(np.sum(w * x * x))
     err = np.abs(got[masks] - ref)
+    well = pmin >= 1e-4                       # class A: the oracle itself is good to ~1e-12 D
+    band = (pmin >= 1e-8) & ~well             # class B: eps / pivot of D is lost on either side
     import os
     os.makedirs("gpurun_out", exist_ok=True)
     with open(os.path.join("gpurun_out", f"subset_alias_{which}.txt"), "w") as fh:
-        fh.write(f"n={n} masks={masks.size} max|dl|/D={err.max() / D:.3e} at mask {int(masks[np.argmax(err)])}\n")
-    assert np.all(np.isfinite(got)) and np.all(got >= 0.0)
-    assert err.max() <= 1e-10 * D, f"max |dl| / D = {err.max() / D:.3e}"
+        for name, sel in (("pivot>=1e-4", well), ("1e-8<=pivot<1e-4", band), ("pivot<1e-8 or dropped", ~well & ~band)):
+            if sel.any():
+                fh.write(f"n={n} {name}: masks={int(sel.sum())} max|dl|/D={err[sel].max() / D:.3e} "
+                         f"max|dl|*pivot/(eps D)={np.max(err[sel] * np.maximum(pmin[sel], 1e-300)) / (2.2e-16 * D):.3e}\n")
+    assert np.all(np.isfinite(got)) and np.all(got >= 0.0) and np.all(got <= got[0] * (1 + 1e-12))
+    assert well.sum() >= masks.size // 8
+    assert err[well].max() <= 1e-10 * D, f"max |dl| / D = {err[well].max() / D:.3e}"
+    if band.any():
+        assert np.all(err[band] <= 1e3 * 2.2e-16 * D / pmin[band])
 
 
 def test_subset_fits_duplicate_frequency_and_errors(fr, p1):
@@ -284,6 +297,74 @@ def test_refine_parity(fr, p1, noise, n):
     f0, l0, it0 = fr.fredec_refine(t, x, w, start, max_iter=0)
     _, l0_ref, _ = p1.refine(t, x, w, start, max_iter=0)
     assert it0 == 0 and np.array_equal(f0, start) and abs(l0 - l0_ref) <= 1e-9 * D
+
+
+def test_refine_batched_parity_1000_tuples(fr, p1):
+    """PAPER.md:214 / :266: the local fits l_{m,loc} of many subsets of one pool in one call (one CTA per
+    tuple, every iteration on the device) against the oracle's refine() looped over the tuples.  Pool: 12
+    frequencies near 12 sinusoids of the series (start values up to 0.2 / T off); 1000 random subsets of
+    1..6 of them + the empty and the full tuple.  Bars: frequencies within 10 tol / T_eff, l within
+    1e-9 D, iteration counts within one (both sides stop on max |step| T_eff <= tol)."""
+    rng = np.random.Generator(np.random.PCG64(2140))
+    N, n_pool = 600, 12
+    t = np.sort(rng.uniform(0.0, 400.0, N))
+    T = t.max() - t.min()
+    f_true = 0.02 + 0.035 * np.arange(n_pool) + rng.uniform(-0.005, 0.005, n_pool)
+    x = 0.4 + sum((3.0 - 0.15 * k) * np.cos(2 * np.pi * f * t + 0.7 * k) for k, f in enumerate(f_true)) \
+        + 0.5 * rng.standard_normal(N)
+    w = rng.uniform(0.5, 2.0, N)
+    pool = f_true + rng.uniform(-0.2, 0.2, n_pool) / T
+    masks = [0, (1 << n_pool) - 1]
+    while len(masks) < 1002:
+        size = int(rng.integers(1, 7))
+        masks.append(int(sum(1 << int(j) for j in rng.choice(n_pool, size=size, replace=False))))
+    masks = np.array(masks, dtype=np.int64)
+    tol = 1e-9
+    freqs, l, iters, status = fr.fredec_refine_batched(t, x, w, pool, masks, max_iter=30, tol=tol)
+    assert np.all(status == 0)
+    T_eff, _ = p1.bandwidth(t, w, 1.0)
+    D = float(np.sum(w * x * x))
+    worst_f = worst_l = 0.0
+    for i, mask in enumerate(masks):
+        sel = [j for j in range(n_pool) if (mask >> j) & 1]
+        f_ref, l_ref, it_ref = p1.refine(t, x, w, pool[sel], max_iter=30, tol=tol)
+        assert abs(int(iters[i]) - it_ref) <= 1, (i, mask, iters[i], it_ref)
+        if sel:
+            worst_f = max(worst_f, float(np.max(np.abs(freqs[i, sel] - f_ref))) * T_eff)
+        worst_l = max(worst_l, abs(l[i] - l_ref))
+        unsel = [j for j in range(n_pool) if not (mask >> j) & 1]
+        assert np.array_equal(freqs[i, unsel], pool[unsel])
+    assert worst_f <= 10 * tol, worst_f
+    assert worst_l <= 1e-9 * D, worst_l / D
+    # the single-tuple call is the batched one with T = 1; device pointers give the same bits
+    import torch
+    f1, l1, it1 = fr.fredec_refine(t, x, w, pool[[1, 4, 7]], max_iter=30, tol=tol)
+    i147 = fr.fredec_refine_batched(t, x, w, pool, np.array([0b10010010]), max_iter=30, tol=tol)
+    assert np.max(np.abs(f1 - i147[0][0, [1, 4, 7]])) * T_eff <= 10 * tol and abs(l1 - i147[1][0]) <= 1e-9 * D
+    fd, ld, _, _ = fr.fredec_refine_batched(*[torch.from_numpy(a).cuda() for a in (t, x, w, pool)], masks[:50],
+                                             max_iter=30, tol=tol)
+    assert np.array_equal(fd, freqs[:50]) and np.array_equal(ld, l[:50])
+    with open("gpurun_out/refine_batched.txt", "w") as fh:
+        tm = fr.fredec_last_timing()
+        fh.write(f"tuples=50 kernel_ms={tm['scan_ms']:.3f}\n")
+    fr.fredec_refine_batched(t, x, w, pool, masks, max_iter=30, tol=tol)
+    with open("gpurun_out/refine_batched.txt", "a") as fh:
+        tm = fr.fredec_last_timing()
+        fh.write(f"tuples={masks.size} N={N} sizes 1..6 (+ empty, full 12): kernel_ms={tm['scan_ms']:.3f} "
+                 f"tuples_per_s={masks.size / (tm['scan_ms'] * 1e-3):.3e}\n")
+
+
+def test_refine_batched_singular_tuple_and_errors(fr):
+    t, x, w, _ = inputs.random_series(2, 80, 0)
+    pool = np.array([0.2, 0.2, 0.31])
+    freqs, l, iters, status = fr.fredec_refine_batched(t, x, w, pool, np.array([0b011, 0b101, 0b100]))
+    assert status.tolist() == [fr.FREDEC_ESINGULAR, 0, 0] and l[0] == 0.0 and l[1] > 0.0
+    with pytest.raises(fr.FredecError):
+        fr.fredec_refine_batched(t, x, w, pool, np.array([8]))                 # bit beyond the pool
+    with pytest.raises(fr.FredecError):
+        fr.fredec_refine_batched(t[:10], x[:10], w[:10], pool, np.array([7]))    # N < 3 m + 2
+    with pytest.raises(fr.FredecError):
+        fr.fredec_refine_batched(t, x, w, np.linspace(0.1, 0.9, 26))           # pool > 25
 
 
 def test_non_finite_frequencies_are_data_errors(fr):
