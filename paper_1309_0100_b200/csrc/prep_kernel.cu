@@ -37,11 +37,14 @@ constexpr int kGramTile = 4;       // a warp accumulates a 4 x 4 block of Gram e
 constexpr int kGramMinSplit = 64;  // observations per warp at least, when a tile's sweep is split between warps
 
 // Shared-memory layout of the prep kernel (doubles), M = d + 1 columns (the base functions and x).
+// `stage` holds the CTA's slice of (w, phi_0 .. phi_{d-1}, x), d + 2 rows of `slice` observations, when it
+// fits: every pass then runs at shared-memory latency and global memory is read and written once.
 struct PrepSmem {
     int M, LD, tiles, splits;
-    size_t part, gram, chol, diag0, stash, scal, total;  // offsets in doubles; total in bytes
+    int64_t slice;  // observations per staged row (0: not staged, the passes run on global memory)
+    size_t part, gram, chol, diag0, scal, stage, total;  // offsets in doubles; total in bytes
 };
-__host__ __device__ inline PrepSmem prep_smem(int d, int splits)
+__host__ __device__ inline PrepSmem prep_smem(int d, int splits, int64_t slice)
 {
     PrepSmem L;
     L.M = d + 1;
@@ -49,13 +52,14 @@ __host__ __device__ inline PrepSmem prep_smem(int d, int splits)
     const int tm = (L.M + kGramTile - 1) / kGramTile;
     L.tiles = tm * (tm + 1) / 2;
     L.splits = splits;
+    L.slice = slice;
     size_t o = 0;
     L.part = o;  o += (size_t)splits * L.tiles * 16;   // per (split, tile): a 4 x 4 block
     L.gram = o;  o += (size_t)L.M * L.LD;              // this CTA's partial Gram matrix (read by the cluster)
     L.chol = o;  o += (size_t)L.M * L.LD;              // the cluster's Gram matrix, factored in place
     L.diag0 = o; o += L.M;
-    L.stash = o; o += (size_t)d * kPrepThreads;        // forward substitution: psi_m of the thread's observation
     L.scal = o;  o += 16;
+    L.stage = o; o += (size_t)(d + 2) * slice;
     L.total = o * sizeof(double);
     return L;
 }
@@ -89,17 +93,25 @@ __device__ double block_min(double v, double* red)
     return r;
 }
 
-// Partial Gram matrix of the columns (rows[0..d-1], xrow) over the observations [i0, i1) of the series:
+// The CTA's view of its slice: rows (w, columns 0 .. d-1, x) with a common stride, in shared memory
+// (staged) or in global memory (then the columns are read from `src`, written to the psi workspace).
+struct Rows {
+    const double* w;
+    double* col;        // column j of observation i: col[j * stride + i]
+    double* x;
+    int64_t stride, n;  // n observations, i = 0 .. n-1
+};
+
+// Partial Gram matrix of the columns (col_0 .. col_{d-1}, x) over the slice:
 // gram[a][b] (a >= b within the tiles of the lower block triangle) = sum_i w_i col_a(i) col_b(i).
 // Work item = (tile, split); a warp sweeps its share of the slice with the lanes striding over the
 // observations and adds the 16 entries over the lanes; the splits are added in fixed order.
-__device__ void gram_partial(const PrepSmem& L, double* sm, const double* __restrict__ w, const double* rows,
-                             const double* xrow, int64_t N, int d, int64_t i0, int64_t i1)
+__device__ void gram_partial(const PrepSmem& L, double* sm, const Rows& R, int d)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int M = L.M;
     double* part = sm + L.part;
-    const int64_t len = i1 - i0, per = (len + L.splits - 1) / L.splits;
+    const int64_t per = (R.n + L.splits - 1) / L.splits;
     for (int item = wid; item < L.tiles * L.splits; item += kPrepWarps) {
         const int tile = item % L.tiles, split = item / L.tiles;
         int ta = 0;
@@ -110,22 +122,24 @@ __device__ void gram_partial(const PrepSmem& L, double* sm, const double* __rest
 #pragma unroll
         for (int j = 0; j < kGramTile; ++j) {
             const int ca = ta * kGramTile + j, cb = tb * kGramTile + j;
-            pa[j] = ca < d ? rows + (int64_t)ca * N : (ca == d ? xrow : nullptr);
-            pb[j] = cb < d ? rows + (int64_t)cb * N : (cb == d ? xrow : nullptr);
+            // columns past x are padding: they read x and are not stored
+            pa[j] = ca < d ? R.col + (int64_t)ca * R.stride : R.x;
+            pb[j] = cb < d ? R.col + (int64_t)cb * R.stride : R.x;
         }
         double acc[kGramTile][kGramTile];
 #pragma unroll
         for (int j = 0; j < kGramTile; ++j)
 #pragma unroll
             for (int k = 0; k < kGramTile; ++k) acc[j][k] = 0.0;
-        const int64_t s0 = i0 + split * per, s1 = min(i1, s0 + per);
+        const int64_t s0 = split * per, s1 = min(R.n, s0 + per);
+#pragma unroll 2
         for (int64_t i = s0 + lane; i < s1; i += 32) {
-            const double wi = w[i];
+            const double wi = R.w[i];
             double va[kGramTile], vb[kGramTile];
 #pragma unroll
             for (int j = 0; j < kGramTile; ++j) {
-                va[j] = pa[j] ? wi * pa[j][i] : 0.0;
-                vb[j] = pb[j] ? pb[j][i] : 0.0;
+                va[j] = wi * pa[j][i];
+                vb[j] = pb[j][i];
             }
 #pragma unroll
             for (int j = 0; j < kGramTile; ++j)
@@ -158,11 +172,19 @@ __device__ void gram_partial(const PrepSmem& L, double* sm, const double* __rest
     }
 }
 
-// chol = sum over the cluster's CTAs, in rank order, of their partial Gram matrices (lower triangles).
-__device__ void gram_cluster_sum(const PrepSmem& L, double* sm, cg::cluster_group& cluster)
+__device__ __forceinline__ void cluster_or_cta_sync(cg::cluster_group& cluster, int C)
 {
-    cluster.sync();  // every CTA's partial matrix is written
-    const int M = L.M, C = (int)cluster.num_blocks();
+    if (C > 1)
+        cluster.sync();
+    else
+        __syncthreads();
+}
+
+// chol = sum over the cluster's CTAs, in rank order, of their partial Gram matrices (lower triangles).
+__device__ void gram_cluster_sum(const PrepSmem& L, double* sm, cg::cluster_group& cluster, int C)
+{
+    cluster_or_cta_sync(cluster, C);  // every CTA's partial matrix is written
+    const int M = L.M;
     double* chol = sm + L.chol;
     for (int e = threadIdx.x; e < M * M; e += kPrepThreads) {
         const int a = e / M, b = e % M;
@@ -172,16 +194,17 @@ __device__ void gram_cluster_sum(const PrepSmem& L, double* sm, cg::cluster_grou
         chol[a * L.LD + b] = v;
         if (a == b) sm[L.diag0 + a] = v;
     }
-    cluster.sync();  // all remote reads done before anyone overwrites its partial matrix
+    cluster_or_cta_sync(cluster, C);  // all remote reads done before anyone overwrites its partial matrix
 }
 
 // In-place Cholesky of the leading d x d block of chol (lower triangle) with row d (the column x) carried
-// along as a right-hand side: afterwards chol[i][j] = L[i][j], chol[d][j] = a_j = (L^{-1} g)_j.
-// Returns false when a pivot^2 <= tau x its original diagonal (dependent base functions, S6b).
+// along as a right-hand side: afterwards chol[i][j] = L[i][j], chol[d][j] = a_j = (L^{-1} g)_j,
+// and diag0[j] = 1 / L[j][j].  Returns false when a pivot^2 <= tau x its original diagonal (dependent base
+// functions, S6b).
 __device__ bool chol_with_x(const PrepSmem& L, double* sm, int d, double tau, int* flag)
 {
     double* S = sm + L.chol;
-    const double* diag0 = sm + L.diag0;
+    double* diag0 = sm + L.diag0;
     const int LD = L.LD, tid = threadIdx.x;
     if (tid == 0) *flag = 0;
     __syncthreads();
@@ -194,6 +217,7 @@ __device__ bool chol_with_x(const PrepSmem& L, double* sm, int d, double tau, in
         const double ljj = sqrt(piv), inv = 1.0 / ljj;
         __syncthreads();
         for (int i = j + tid; i <= d; i += kPrepThreads) S[i * LD + j] = i == j ? ljj : S[i * LD + j] * inv;
+        if (tid == 0) diag0[j] = inv;  // the original diagonal of column j is not needed again
         __syncthreads();
         const int rows = d - j;  // rows j+1 .. d, columns j+1 .. min(row, d-1)
         for (int e = tid; e < rows * rows; e += kPrepThreads) {
@@ -207,30 +231,30 @@ __device__ bool chol_with_x(const PrepSmem& L, double* sm, int d, double tau, in
 }
 
 // psi_j(i) = (phi_j(i) - sum_{m<j} L[j][m] psi_m(i)) / L[j][j],  x'(i) = x(i) - sum_j a_j psi_j(i), one
-// thread per observation of [i0, i1); src / xsrc may alias dst / xdst (a thread touches its own column only).
-__device__ void apply_factor(const PrepSmem& L, double* sm, int d, const double* src, const double* xsrc, double* dst,
-                             double* xdst, int64_t N, int64_t i0, int64_t i1)
+// thread per observation of the slice; `src` columns (stride src_stride) are read, R.col / R.x written
+// (they may be the same memory: a thread touches its own observation only, and reads back its own writes).
+__device__ void apply_factor(const PrepSmem& L, double* sm, int d, const double* src, int64_t src_stride,
+                             const double* xsrc, const Rows& R)
 {
     const double* S = sm + L.chol;
-    double* stash = sm + L.stash + threadIdx.x;
+    const double* inv = sm + L.diag0;
     const int LD = L.LD;
-    for (int64_t i = i0 + threadIdx.x; i < i1; i += kPrepThreads) {
+    for (int64_t i = threadIdx.x; i < R.n; i += kPrepThreads) {
         double xv = xsrc[i];
         for (int j = 0; j < d; ++j) {
-            double v = src[(int64_t)j * N + i];
+            double v = src[(int64_t)j * src_stride + i];
             const double* row = S + j * LD;
-            for (int m = 0; m < j; ++m) v = fma(-row[m], stash[m * kPrepThreads], v);
-            v /= row[j];
-            stash[j * kPrepThreads] = v;
-            dst[(int64_t)j * N + i] = v;
+            for (int m = 0; m < j; ++m) v = fma(-row[m], R.col[(int64_t)m * R.stride + i], v);
+            v *= inv[j];
+            R.col[(int64_t)j * R.stride + i] = v;
             xv = fma(-S[d * LD + j], v, xv);
         }
-        xdst[i] = xv;
+        R.x[i] = xv;
     }
     __syncthreads();
 }
 
-__global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p, int splits)
+__global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p, int splits, int64_t slice)
 {
     extern __shared__ __align__(16) double sm[];
     __shared__ double red[32];
@@ -239,27 +263,43 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p, int sp
     const int C = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
     const int64_t b = blockIdx.y, N = p.N;
     const int d = p.d;
-    const PrepSmem L = prep_smem(d, splits);
-    const double* t = p.t + b * N;
-    const double* x = p.x + b * N;
-    const double* w = p.w + b * N;
-    const double* base = p.base ? p.base + b * (int64_t)d * N : nullptr;
-    double* psi = p.psi + b * (int64_t)d * N;  // [d][N]
-    double* xt = p.xt + b * N;                 // [N]
-    SeriesInfo* info = p.info + b;
+    const PrepSmem L = prep_smem(d, splits, slice);
     const int64_t i0 = N * rank / C, i1 = N * (rank + 1) / C;  // this CTA's observations
+    const double* t = p.t + b * N + i0;
+    const double* x = p.x + b * N + i0;
+    const double* w = p.w + b * N + i0;
+    const double* base = p.base ? p.base + b * (int64_t)d * N + i0 : nullptr;
+    double* psi = p.psi + b * (int64_t)d * N + i0;  // [d][N]
+    double* xt = p.xt + b * N + i0;                 // [N]
+    SeriesInfo* info = p.info + b;
     double* scal = sm + L.scal;
+    const bool staged = slice > 0;
+    Rows R;
+    R.n = i1 - i0;
+    R.stride = staged ? slice : N;
+    R.w = staged ? sm + L.stage : w;
+    R.col = staged ? sm + L.stage + slice : psi;
+    R.x = staged ? sm + L.stage + (d + 1) * slice : xt;
 
-    // ---- a1: validate, W = <1>, time origin --------------------------------------------
+    // ---- a1: validate, W = <1>, time origin; the slice goes to shared memory when it fits -----------
     double bad = 0.0, wsum = 0.0, tmin = INFINITY, tmax = -INFINITY;
-    for (int64_t i = i0 + threadIdx.x; i < i1; i += kPrepThreads) {
+    for (int64_t i = threadIdx.x; i < R.n; i += kPrepThreads) {
         const double ti = t[i], xi = x[i], wi = w[i];
         if (!isfinite(ti) || !isfinite(xi) || !isfinite(wi) || wi < 0.0) bad = 1.0;
         wsum += wi;
         tmin = fmin(tmin, ti);
         tmax = fmax(tmax, ti);
-        for (int j = 0; j < d; ++j)
-            if (!isfinite(base[(int64_t)j * N + i])) bad = 1.0;
+        if (staged) {
+            sm[L.stage + i] = wi;
+            R.x[i] = xi;
+        }
+    }
+    // the base functions as one flat sweep (independent loads, whole rows back to back)
+    for (int64_t e = threadIdx.x; e < (int64_t)d * R.n; e += kPrepThreads) {
+        const int64_t j = e / R.n, i = e - j * R.n;
+        const double v = base[j * N + i];
+        if (!isfinite(v)) bad = 1.0;
+        if (staged) R.col[j * slice + i] = v;
     }
     bad = block_sum(bad, red);
     wsum = block_sum(wsum, red);
@@ -271,7 +311,7 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p, int sp
         scal[2] = tmin;
         scal[3] = tmax;
     }
-    cluster.sync();
+    cluster_or_cta_sync(cluster, C);
     double W = 0.0;
     bad = 0.0;
     tmin = INFINITY;
@@ -291,22 +331,33 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p, int sp
     // (with invalid data the passes run on whatever is there and the results are ignored: no CTA may
     // leave the cluster's barriers)
     for (int pass = 0; pass < 2; ++pass) {
-        const double* src = pass == 0 ? base : psi;
-        const double* xsrc = pass == 0 ? x : xt;
-        gram_partial(L, sm, w, src, xsrc, N, d, i0, i1);
-        gram_cluster_sum(L, sm, cluster);
+        // not staged: the first pass reads the caller's base functions and x, and writes the workspace
+        Rows G = R;
+        if (!staged && pass == 0) {
+            G.col = const_cast<double*>(base);
+            G.x = const_cast<double*>(x);
+        }
+        gram_partial(L, sm, G, d);
+        gram_cluster_sum(L, sm, cluster, C);
         // pass 0 decides whether the base functions are dependent (S6b); pass 1 factors a matrix
         // that is the identity up to the first pass's orthogonality error
         const bool ok = chol_with_x(L, sm, d, pass == 0 ? kTauBase : 0.0, &flag);
         if (!ok && status == 0) status = -3;  // FREDEC_ESINGULAR (the same decision in every CTA)
-        if (ok) apply_factor(L, sm, d, src, xsrc, psi, xt, N, i0, i1);
+        if (ok) apply_factor(L, sm, d, G.col, G.stride, G.x, R);
     }
     double chi2 = 0.0;
-    for (int64_t i = i0 + threadIdx.x; i < i1; i += kPrepThreads) chi2 = fma(w[i] * xt[i], xt[i], chi2);
+    for (int64_t i = threadIdx.x; i < R.n; i += kPrepThreads) chi2 = fma(R.w[i] * R.x[i], R.x[i], chi2);
     chi2 = block_sum(chi2, red);
-    cluster.sync();  // the a1 scalars have been read by every CTA
+    if (staged) {  // results to the workspace: whole rows, coalesced
+        for (int64_t e = threadIdx.x; e < (int64_t)d * R.n; e += kPrepThreads) {
+            const int64_t j = e / R.n, i = e - j * R.n;
+            psi[j * N + i] = R.col[j * slice + i];
+        }
+        for (int64_t i = threadIdx.x; i < R.n; i += kPrepThreads) xt[i] = R.x[i];
+    }
+    cluster_or_cta_sync(cluster, C);  // the a1 scalars have been read by every CTA
     if (threadIdx.x == 0) scal[0] = chi2;
-    cluster.sync();
+    cluster_or_cta_sync(cluster, C);
     if (rank == 0 && threadIdx.x == 0) {
         double total = 0.0;
         for (int r = 0; r < C; ++r) total += cluster.map_shared_rank(scal, r)[0];
@@ -316,27 +367,29 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p, int sp
         info->status = status;
         info->pad = 0;
     }
-    cluster.sync();  // no CTA exits while its shared memory may still be read
+    cluster_or_cta_sync(cluster, C);  // no CTA exits while its shared memory may still be read
 }
 
 // ---- a3: per-observation table and seed records --------------------------
-// One thread per observation (padded to whole groups of 4 with zero multipliers).  Layout:
-// scan_mma_kernel.cuh.
-constexpr int kTableThreads = 128;
+// One thread per (observation, pair of column tiles tp, position hh in a tile): two grid offsets h and h + 4,
+// four sincospi of exactly reduced phases, and the entries of every family for them.  The series are
+// padded to whole groups of 4 observations with zero multipliers.  Layout: scan_mma_kernel.cuh.
+constexpr int kTableObs = 32;  // observations per CTA (threadIdx.x); threadIdx.y = tp * 4 + hh
 
-__global__ void __launch_bounds__(kTableThreads) table_kernel(TableParams p)
+__global__ void table_kernel(TableParams p)
 {
     const int64_t b = blockIdx.z, N = p.N;
     const int pass = blockIdx.y;
     const SeriesInfo info = p.info[b];
     if (info.status != 0) return;
-    const int64_t i = (int64_t)blockIdx.x * kTableThreads + threadIdx.x;
+    const int64_t i = (int64_t)blockIdx.x * kTableObs + threadIdx.x;
     if (i >= p.G4 * 4) return;
     const bool real = i < N;
     const int H = p.H, NT = mma_nt(H), NF = mma_nf(p.NB);
+    const int tp = threadIdx.y >> 2, hh = threadIdx.y & 3;
     const double tc = real ? p.t[b * N + i] - info.t_mid : 0.0;
     const double wi = real ? p.w[b * N + i] : 0.0;
-    if (pass == 0) {
+    if (pass == 0 && threadIdx.y == 0) {
         SeedRec r;
         r.t = tc;
         sincospi(2.0 * frac_prod(p.df * (double)(16 * H), tc), &r.su, &r.cu);  // one unit = 8 runs of 2H steps
@@ -349,33 +402,30 @@ __global__ void __launch_bounds__(kTableThreads) table_kernel(TableParams p)
     const double* psi = p.psi + b * (int64_t)p.d * N;
     // column tiles are stored in pairs (one 16-byte load per lane fetches the fragments of two): the
     // thread writes the entries of tiles 2 tp and 2 tp + 1, i.e. of h and h + 4, as one double2
-    for (int tp = 0; tp < NT / 2; ++tp) {
-        for (int hh = 0; hh < 4; ++hh) {
-            double c1[2], s1[2], c2[2], s2[2];
-            for (int e = 0; e < 2; ++e) {
-                const int h = 8 * tp + 4 * e + hh + 1;
-                // alpha_h = 2 pi (h - 1/2) df t' in turns, range-reduced exactly
-                const double x = frac_prod((double)(2 * h - 1) * (0.5 * p.df), tc);
-                sincospi(2.0 * x, &s1[e], &c1[e]);
-                sincospi(4.0 * x, &s2[e], &c2[e]);
-            }
-            const int n0 = 2 * hh;
-            for (int f = 0; f < NF; ++f) {
-                double m;
-                const bool dbl = f == NF - 1;  // the w family uses the doubled angles
-                if (f == 0) {
-                    m = (pass == 0 && real) ? wi * p.xt[b * N + i] : 0.0;
-                } else if (dbl) {
-                    m = pass == 0 ? 0.5 * wi : 0.0;
-                } else {
-                    const int j = pass * p.NB + (f - 1);
-                    m = (j < p.d && real) ? wi * psi[(int64_t)j * N + i] : 0.0;
-                }
-                double2* tile = reinterpret_cast<double2*>(grp + (f * (NT / 2) + tp) * 64);
-                tile[n0 * 4 + k] = make_double2(m * (dbl ? c2[0] : c1[0]), m * (dbl ? c2[1] : c1[1]));
-                tile[(n0 + 1) * 4 + k] = make_double2(m * (dbl ? s2[0] : s1[0]), m * (dbl ? s2[1] : s1[1]));
-            }
+    double c1[2], s1[2], c2[2], s2[2];
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+        const int h = 8 * tp + 4 * e + hh + 1;
+        // alpha_h = 2 pi (h - 1/2) df t' in turns, range-reduced exactly
+        const double x = frac_prod((double)(2 * h - 1) * (0.5 * p.df), tc);
+        sincospi(2.0 * x, &s1[e], &c1[e]);
+        sincospi(4.0 * x, &s2[e], &c2[e]);
+    }
+    const int n0 = 2 * hh;
+    for (int f = 0; f < NF; ++f) {
+        double m;
+        const bool dbl = f == NF - 1;  // the w family uses the doubled angles
+        if (f == 0) {
+            m = (pass == 0 && real) ? wi * p.xt[b * N + i] : 0.0;
+        } else if (dbl) {
+            m = pass == 0 ? 0.5 * wi : 0.0;
+        } else {
+            const int j = pass * p.NB + (f - 1);
+            m = (j < p.d && real) ? wi * psi[(int64_t)j * N + i] : 0.0;
         }
+        double2* tile = reinterpret_cast<double2*>(grp + (f * (NT / 2) + tp) * 64);
+        tile[n0 * 4 + k] = make_double2(m * (dbl ? c2[0] : c1[0]), m * (dbl ? c2[1] : c1[1]));
+        tile[(n0 + 1) * 4 + k] = make_double2(m * (dbl ? s2[0] : s1[0]), m * (dbl ? s2[1] : s1[1]));
     }
 }
 
@@ -383,23 +433,28 @@ __global__ void __launch_bounds__(kTableThreads) table_kernel(TableParams p)
 
 cudaError_t launch_table(const TableParams& p, int64_t B, cudaStream_t stream)
 {
-    dim3 grid((unsigned)((p.G4 * 4 + kTableThreads - 1) / kTableThreads), (unsigned)p.n_pass, (unsigned)B);
-    table_kernel<<<grid, kTableThreads, 0, stream>>>(p);
+    dim3 grid((unsigned)((p.G4 * 4 + kTableObs - 1) / kTableObs), (unsigned)p.n_pass, (unsigned)B);
+    dim3 block(kTableObs, (unsigned)(mma_nt(p.H) / 2 * 4));  // at most 32 x 24 threads (H = 48)
+    table_kernel<<<grid, block, 0, stream>>>(p);
     return cudaGetLastError();
 }
 
 cudaError_t launch_prep(const PrepParams& p, int64_t B, cudaStream_t stream)
 {
-    // CTAs per series: one per ~16k input values, at most 8 (a portable cluster), one when there are many series
+    // CTAs per series (a thread-block cluster, at most 8): as few as let the slice of (w, base, x) sit in
+    // shared memory beside the matrices, one when there are many series
+    constexpr size_t kSmemMax = 220 * 1024;
+    const size_t fixed = prep_smem(p.d, kPrepWarps, 0).total;
     int C = 1;
+    auto fits = [&](int c) { return fixed + (size_t)(p.d + 2) * ((p.N + c - 1) / c) * 8 <= kSmemMax; };
     if (B <= 64)
-        while (C < kPrepMaxCluster && (int64_t)p.N * (p.d + 2) > (int64_t)16384 * C) C *= 2;
-    const int64_t slice = (p.N + C - 1) / C;
-    const PrepSmem probe = prep_smem(p.d, 1);
-    int splits = kPrepWarps / probe.tiles;
-    if (splits > (int)(slice / kGramMinSplit)) splits = (int)(slice / kGramMinSplit);
+        while (C < kPrepMaxCluster && !fits(C)) C *= 2;
+    const int64_t per_cta = (p.N + C - 1) / C;
+    const int64_t slice = fits(C) ? per_cta : 0;
+    int splits = kPrepWarps / prep_smem(p.d, 1, 0).tiles;
+    if (splits > (int)(per_cta / kGramMinSplit)) splits = (int)(per_cta / kGramMinSplit);
     if (splits < 1) splits = 1;
-    const PrepSmem L = prep_smem(p.d, splits);
+    const PrepSmem L = prep_smem(p.d, splits, slice);
     static size_t attr_smem = 0;
     if (L.total > attr_smem) {
         cudaError_t e = cudaFuncSetAttribute(prep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total);
@@ -418,7 +473,7 @@ cudaError_t launch_prep(const PrepParams& p, int64_t B, cudaStream_t stream)
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, prep_kernel, p, splits);
+    return cudaLaunchKernelEx(&cfg, prep_kernel, p, splits, slice);
 }
 
 }  // namespace fredec

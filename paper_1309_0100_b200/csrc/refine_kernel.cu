@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(kRefThreads) refine_batched_kernel(RefineParam
     __syncthreads();
 
     int iters = 0, status = p.bw[3] != 0.0 || !(T_eff > 0.0) ? -2 : 0;
-    bool converged = p.max_iter == 0;
+    bool converged = p.max_iter == 0 || m == 0;  // the empty tuple has nothing to iterate
     double l = 0.0;
     while (status == 0) {
         // ---- Gram matrix of the extended rows, one sweep over the observations ----------------

@@ -512,14 +512,16 @@ __device__ __forceinline__ double solve_z(double YC, double YS, double CC, doubl
 {
     const double SS = W - CC;  // <sin^2> = <1> - <cos^2>
     const double Scc = CC - Saa, Scs = CS - Sab, Sss = SS - Sbb;
+    // two reciprocals instead of three divisions: the epilogue's FP64 instructions run while no MMA does
     double z = 0.0, ys = YS, piv2 = Sss;
     if (Scc > kTauTrial * CC) {  // S6: otherwise the cos column is in the span of the base
-        const double q = Scs / Scc;
-        z = YC * YC / Scc;
+        const double r = 1.0 / Scc;
+        const double q = Scs * r;
+        z = YC * YC * r;
         ys = fma(-q, YC, YS);
         piv2 = fma(-q, Scs, Sss);
     }
-    if (piv2 > kTauTrial * SS) z = fma(ys, ys / piv2, z);
+    if (piv2 > kTauTrial * SS) z = fma(ys * ys, 1.0 / piv2, z);
     return z;
 }
 

@@ -244,7 +244,7 @@ def test_host_and_device_pointers_agree_bitwise(fr):
     assert np.array_equal(za, zb) and np.array_equal(za, zc)      # also: run-to-run reproducible
 
 
-@pytest.mark.parametrize("N,d", [(600, 9), (2000, 51), (5000, 2), (20_000, 33), (3000, 64), (70, 64)])
+@pytest.mark.parametrize("N,d", [(600, 9), (2000, 51), (5000, 2), (20_000, 33), (3000, 64), (150, 64)])
 def test_prep_cluster_sizes_and_base_fit(fr, oracle_mod, N, d):
     """Rows a1/a2 (base orthogonalisation by two passes of Cholesky QR, one thread-block cluster per
     series): sizes that run on 1, 2, 4 and 8 CTAs per series, up to FREDEC_D_MAX functions.  chi2_base
@@ -259,6 +259,22 @@ def test_prep_cluster_sizes_and_base_fit(fr, oracle_mod, N, d):
     z = gpu_scan(fr, t, x, w, base, f0, df, K)
     assert_parity(z, z_ref, f"N={N},d={d}")
     assert np.array_equal(z, gpu_scan(fr, t, x, w, base, f0, df, K))
+
+
+def test_prep_ill_conditioned_base_against_qr(fr, oracle_mod):
+    """64 functions on 70 points: the weighted design matrix has condition 3e6.  The oracle solves the
+    normal equations, which loses cond^2 eps ~ 1e-3 of chi2_base here (its FP64 result is
+    9e-6 off), so this case is held against the Householder-QR least squares that pins the oracle
+    (tests/test_oracle_pins.py) and against the oracle's 80-bit build, not against the FP64 oracle."""
+    N, d = 70, 64
+    t, x, w, base = inputs.random_series(5000 + N + d, N, d, t_span=400.0)
+    A = (base * np.sqrt(w)).T
+    theta = np.linalg.lstsq(A, np.sqrt(w) * x, rcond=None)[0]
+    r = np.sqrt(w) * x - A @ theta
+    chi2_qr = float(r @ r)
+    chi2 = fr.fredec_chi2_base(t, x, w, base)
+    assert abs(chi2 - chi2_qr) <= 1e-9 * chi2_qr
+    assert abs(chi2 - oracle_mod.chi2_base(t, x, w, base, long_double=True)) <= 1e-7 * chi2_qr
 
 
 def test_prep_dependent_base_is_singular(fr):

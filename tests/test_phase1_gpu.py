@@ -299,7 +299,7 @@ def test_refine_parity(fr, p1, noise, n):
     assert it0 == 0 and np.array_equal(f0, start) and abs(l0 - l0_ref) <= 1e-9 * D
 
 
-def test_refine_batched_parity_1000_tuples(fr, p1):
+def test_refine_batched_parity_1000_tuples(fr, p1, oracle_mod):
     """PAPER.md:214 / :266: the local fits l_{m,loc} of many subsets of one pool in one call (one CTA per
     tuple, every iteration on the device) against the oracle's refine() looped over the tuples.  Pool: 12
     frequencies near 12 sinusoids of the series (start values up to 0.2 / T off); 1000 random subsets of
@@ -327,6 +327,9 @@ def test_refine_batched_parity_1000_tuples(fr, p1):
     worst_f = worst_l = 0.0
     for i, mask in enumerate(masks):
         sel = [j for j in range(n_pool) if (mask >> j) & 1]
+        if not sel:                        # the empty tuple: the constant alone, nothing to iterate
+            assert iters[i] == 0 and abs(l[i] - oracle_mod.chi2_base(t, x, w, np.ones((1, N)))) <= 1e-12 * D
+            continue
         f_ref, l_ref, it_ref = p1.refine(t, x, w, pool[sel], max_iter=30, tol=tol)
         assert abs(int(iters[i]) - it_ref) <= 1, (i, mask, iters[i], it_ref)
         if sel:
