@@ -42,9 +42,11 @@ FP64_LANES_PER_SM = 64
 L2_FLUSH_BYTES = 256 << 20
 ORACLE_SAMPLE_K = 100_000         # grid points of config 4 the CPU legs time per step (~20 core-seconds)
 # dram__bytes_read.sum + dram__bytes_write.sum of one scan_mma_kernel launch on config 4, from the
-# `ncu --set full` capture summarised in profiles/r1_scan_mma_kernel_ncu.md (read only: the 16 MB
-# periodogram is still in L2 when the kernel ends).  Algorithmic bytes: 10.6 MB table + 16 MB z.
-SCAN_DRAM_TRAFFIC_BYTES = 11_000_000
+# `ncu --set full` capture summarised in the file named below -- NOT measured in the bench run (ncu
+# cannot run inside it).  Algorithmic bytes: table + seed records + 16 MB z (the periodogram is still
+# in L2 when the kernel ends, so the capture sees less than that).
+SCAN_DRAM_TRAFFIC_BYTES = 12_090_112
+SCAN_DRAM_TRAFFIC_SOURCE = "profiles/r1_scan_mma_kernel_ncu.md (ncu --set full capture; not measured in this run)"
 
 
 def flops_per_pair(d: int) -> int:
@@ -416,6 +418,7 @@ def main_ours(args):
         "fraction_of_fp64_peak_rotation_form_equivalent": achieved / peak_nominal * (15 + 4 * wl.d) / F,
         "roofline": {"bound": "alu", "kernel": "scan_mma_kernel", "achieved": achieved, "peak": peak_nominal,
                      "unit": "TFLOP/s", "frac": achieved / peak_nominal, "traffic": SCAN_DRAM_TRAFFIC_BYTES,
+                     "traffic_source": SCAN_DRAM_TRAFFIC_SOURCE,
                      "flops_per_pair": F, "peak_source": f"nominal: {sm_count} SMs x {FP64_LANES_PER_SM} FP64 FMA "
                      "lanes x 2 x 1.965 GHz (DESIGN.md section 6)",
                      "peak_measured_dfma": peak_tf, "frac_of_measured_dfma": achieved / peak_tf},
@@ -466,6 +469,47 @@ def main_fp64_probe(args):
     return 0
 
 
+def main_profile(args):
+    """`--profile-config N`: runs only the hot path of workload N (warm-up + steps calls) and prints
+    its per-kernel device times: the command the ncu captures under profiles/ wrap (one workload per
+    process, so that `ncu -k ... -s ... -c 1` picks a known launch)."""
+    import torch
+    from paper_1309_0100_b200 import build as lib_build
+    lib_build.build()
+    import paper_1309_0100_b200 as fr
+    from paper_1309_0100_b200 import inputs
+    torch.cuda.set_device(0)
+    stream = torch.cuda.current_stream()
+    fr.fredec_set_stream(stream)
+    kw = {}
+    if args.profile_n:
+        kw["N"] = args.profile_n
+    if args.profile_k:
+        kw["K"] = args.profile_k
+    if args.profile_nbase:
+        kw["n_base"] = args.profile_nbase
+    wl = inputs.config(args.profile_config, **kw)
+    batched = wl.B > 1
+    arrs = (wl.t, wl.x, wl.w, wl.base_funcs) if batched else wl.series(0)
+    d_in = [torch.from_numpy(a).cuda() for a in arrs]
+    z = None if args.profile_no_z else torch.empty((wl.B, wl.K) if batched else wl.K, dtype=torch.float64, device="cuda")
+    idx = torch.empty((wl.B, wl.topk) if batched else wl.topk, dtype=torch.int64, device="cuda")
+    call = fr.fredec_scan_topk_batched if batched else fr.fredec_scan_topk
+    best = None
+    for i in range(args.warmup + args.steps):
+        call(*d_in, wl.f0, wl.df, wl.K, wl.topk, z_out=z, idx_out=idx, want_z=not args.profile_no_z)
+        tm = fr.fredec_last_timing()
+        if i >= args.warmup and (best is None or tm["total_ms"] < best["total_ms"]):
+            best = tm
+    F = flops_per_pair(wl.d)
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    print(json.dumps({"workload": f"{wl.name}: B={wl.B} N={wl.N} K={wl.K} d={wl.d} top-{wl.topk}",
+                      "z_out": not args.profile_no_z, "kernel_ms": best, "launches": fr.fredec_last_launches(),
+                      "scan_fraction_of_fp64_peak": wl.pairs * F / (best["scan_ms"] * 1e-3) / 1e12
+                      / (sms * FP64_LANES_PER_SM * 2 * 1.965e-3)}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -476,11 +520,19 @@ def main():
     ap.add_argument("--no-multi-series", action="store_true", help="skip the config-5 side measurement")
     ap.add_argument("--no-small-configs", action="store_true", help="skip the configs 1-3 block")
     ap.add_argument("--fp64-probe", action="store_true", help="run the FP64 roofline probes and exit")
+    ap.add_argument("--profile-config", type=int, default=0, choices=[0, 1, 2, 3, 4, 5],
+                    help="run only workload N's hot path (for ncu captures) and exit")
+    ap.add_argument("--profile-n", type=int, default=0, help="with --profile-config: override N")
+    ap.add_argument("--profile-k", type=int, default=0, help="with --profile-config: override K")
+    ap.add_argument("--profile-nbase", type=int, default=0, help="with --profile-config 3: sinusoids in the base")
+    ap.add_argument("--profile-no-z", action="store_true", help="with --profile-config: peaks only (z_out = NULL)")
     args = ap.parse_args()
     if args.steps < 1:
         ap.error("--steps must be >= 1")
     if args.fp64_probe:
         return main_fp64_probe(args)
+    if args.profile_config:
+        return main_profile(args)
     return main_reference(args) if args.impl == "reference" else main_ours(args)
 
 

@@ -134,11 +134,15 @@ def rv_like(N: int = 1000, K: int = 80_000) -> Workload:
                    signal_periods=list(RV_PERIODS), phases=phases.tolist())
 
 
-def residual(N: int = 2000, K: int = 200_000) -> Workload:
+def residual(N: int = 2000, K: int = 200_000, n_base: int = 4) -> Workload:
+    """n_base accepted sinusoids in the base model (d = 2 n_base + 1): the first four signal periods,
+    then -- for the late SLICK iterations of PAPER.md:208-210, whose base reaches d = 51 -- further
+    fixed periods 3.7 * 1.31^j d."""
     t, x, w, phases = _rv_series(_rng(3), N)
-    base = base_offset_sinusoids(t, RV_PERIODS[:4])
+    periods = list(RV_PERIODS[:4]) + [3.7 * 1.31**j for j in range(max(0, n_base - 4))]
+    base = base_offset_sinusoids(t, periods[:n_base])
     return _single("residual", t, x, w, base, 1e-4, 1e-5, K, 10,
-                   signal_periods=list(RV_PERIODS), base_periods=list(RV_PERIODS[:4]),
+                   signal_periods=list(RV_PERIODS), base_periods=periods[:n_base],
                    phases=phases.tolist())
 
 
