@@ -13,7 +13,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libfredec_b200.so")
+# FREDEC_LIB: a measurement build of the same library (paper_1309_0100_b200/build.py --variant), for A/B timings
+LIB_PATH = os.environ.get("FREDEC_LIB") or os.path.join(_HERE, "libfredec_b200.so")
 
 FREDEC_OK, FREDEC_EINVAL, FREDEC_EDATA, FREDEC_ESINGULAR, FREDEC_ECUDA = 0, -1, -2, -3, -4
 FREDEC_D_MAX, FREDEC_TOPK_MAX = 64, 1024

@@ -1,5 +1,10 @@
 """Build libfredec_b200.so (the C-ABI library of include/fredec.h) in-tree with nvcc for
-sm_100a.  `python -m paper_1309_0100_b200.build [--force]`.  nvcc cross-compiles without a GPU."""
+sm_100a.  `python -m paper_1309_0100_b200.build [--force]`.  nvcc cross-compiles without a GPU.
+
+Measurement builds: `python -m paper_1309_0100_b200.build --variant NAME -DMACRO[=V] ...` compiles the
+same sources with extra macros (the FREDEC_EXP_* switches documented where they appear in csrc/) into
+libfredec_b200.NAME.so beside the product library; `FREDEC_LIB=<path>` makes the binding load it.  Such a
+library is for A/B timings only (profiles/r2_experiments.md): some switches give wrong results."""
 from __future__ import annotations
 
 import os
@@ -31,16 +36,18 @@ def _newest_header() -> float:
     return max(os.path.getmtime(h) for h in hs)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    os.makedirs(OBJ, exist_ok=True)
+def build(force: bool = False, verbose: bool = False, variant: str = "", defines=()) -> str:
+    obj_dir = OBJ if not variant else os.path.join(OBJ, "variant_" + variant)
+    lib_path = LIB if not variant else os.path.join(PKG, f"libfredec_b200.{variant}.so")
+    os.makedirs(obj_dir, exist_ok=True)
     nvcc = _nvcc()
     hdr = _newest_header()
     jobs = []
     for src in SOURCES:
         s = os.path.join(CSRC, src)
-        o = os.path.join(OBJ, src.replace(".cu", ".o"))
-        if force or not os.path.exists(o) or os.path.getmtime(o) < max(os.path.getmtime(s), hdr):
-            jobs.append([nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-c", s, "-o", o])
+        o = os.path.join(obj_dir, src.replace(".cu", ".o"))
+        if force or variant or not os.path.exists(o) or os.path.getmtime(o) < max(os.path.getmtime(s), hdr):
+            jobs.append([nvcc, *NVCC_FLAGS, *defines, *(["-Xptxas", "-v"] if verbose else []), "-c", s, "-o", o])
 
     def run(cmd):
         r = subprocess.run(cmd, capture_output=True, text=True)
@@ -53,11 +60,13 @@ def build(force: bool = False, verbose: bool = False) -> str:
             for out in ex.map(run, jobs):
                 if verbose and out:
                     print(out, file=sys.stderr)
-    objs = [os.path.join(OBJ, s.replace(".cu", ".o")) for s in SOURCES]
-    if jobs or not os.path.exists(LIB):
-        run([nvcc, "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a"])
-    return LIB
+    objs = [os.path.join(obj_dir, s.replace(".cu", ".o")) for s in SOURCES]
+    if jobs or not os.path.exists(lib_path):
+        run([nvcc, "-shared", "-o", lib_path, *objs, "-gencode", "arch=compute_100a,code=sm_100a"])
+    return lib_path
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    _variant = sys.argv[sys.argv.index("--variant") + 1] if "--variant" in sys.argv else ""
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, variant=_variant,
+                defines=[a for a in sys.argv[1:] if a.startswith("-D")]))

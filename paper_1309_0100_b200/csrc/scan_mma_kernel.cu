@@ -374,8 +374,8 @@ __device__ __forceinline__ void mma_group_pipelined(Tiles<H, 1, NB>& acc, LoadPi
 }
 
 // The loads of a group's successor are issued whether or not there is one (no selects in the loop): past
-// the last group of a slot they read the slot's own seed area, the next slot, or the kPipePad bytes the
-// launch adds behind the ring, and the values are not used.
+// the last group of a slot they read the next table tile / seed block of the ring or the kPipePad bytes
+// the launch adds behind it, and the values are not used.
 constexpr int kPipePad = 8192;
 
 template <int H, int NB>
@@ -388,6 +388,8 @@ __device__ __forceinline__ void round_mma_pipelined(Tiles<H, 1, NB>& acc, RingPo
     constexpr uint32_t GROUP_B = NF * NT * 32 * 8, SEED_B = CAP * 32 * 16;  // bytes per group: table, seeds
     static_assert(SEED_B + 16 <= kPipePad && (D - 1) * 512 <= kPipePad, "padding behind the ring too small");
     const int64_t g_end = min((int64_t)tile1 * KS, G4);
+    const uint32_t seed_slot = (uint32_t)(slot_bytes - tab_bytes);
+    const uint32_t tab_ring = smem_u32(smem), seed_ring = tab_ring + NS * (uint32_t)tab_bytes;
 #pragma unroll 1
     for (int64_t g = (int64_t)tile0 * KS; g < g_end; g += KS) {
         const int ngrp = (int)min((int64_t)KS, g_end - g);
@@ -395,20 +397,21 @@ __device__ __forceinline__ void round_mma_pipelined(Tiles<H, 1, NB>& acc, RingPo
             mbar_wait(&bar_tab[rp.slot], rp.par);
             mbar_wait(&bar_seed[rp.slot], rp.par);
         }
-        const uint32_t base = smem_u32(smem + rp.slot * slot_bytes);
         int nslot = rp.slot + 1;
         uint32_t npar = rp.par;
         if (nslot == NS) {
             nslot = 0;
             npar ^= 1u;
         }
-        uint32_t tk = base + lane * 16;
-        uint32_t sk = base + (uint32_t)tab_bytes + (role.off * 32 + lane) * 16;
+        uint32_t tk = tab_ring + rp.slot * (uint32_t)tab_bytes + lane * 16;
+        uint32_t sk = seed_ring + rp.slot * seed_slot + (role.off * 32 + lane) * 16;
         rp.ready = false;
         LoadPipe<D> lp;
         if (role.S == 1) {
             // every group of the slot, two per iteration; the next slot's barriers are looked at two or
-            // three groups before the end, so that the MMA stream continues across slots
+            // three groups before the end, so that the MMA stream continues across slots.  (The load
+            // pipeline restarts in every slot: carrying it across the slot boundary was measured and is
+            // slower -- profiles/r2_experiments.md.)
             lp.a = lds128(sk);
 #pragma unroll
             for (int q = 0; q < D - 1; ++q) lp.b[q] = lds128(tk + q * 512);
@@ -466,9 +469,10 @@ __device__ __forceinline__ void round_mma(Tiles<H, NOCT, NB>& acc, RingPos& rp, 
             mbar_wait(&bar_tab[rp.slot], rp.par);
             mbar_wait(&bar_seed[rp.slot], rp.par);
         }
-        const unsigned char* base = smem + rp.slot * slot_bytes;
-        const double2* tk = reinterpret_cast<const double2*>(base) + lane;  // this lane's table fragments
-        const double2* sk = reinterpret_cast<const double2*>(base + tab_bytes) + (size_t)role.off * 32 + lane;
+        // ring layout: the NS table tiles, then the NS seed blocks
+        const double2* tk = reinterpret_cast<const double2*>(smem + rp.slot * tab_bytes) + lane;  // this lane's table fragments
+        const double2* sk = reinterpret_cast<const double2*>(smem + NS * tab_bytes + rp.slot * (slot_bytes - tab_bytes)) +
+                            (size_t)role.off * 32 + lane;
         int nslot = rp.slot + 1;
         uint32_t npar = rp.par;
         if (nslot == NS) {
@@ -632,7 +636,18 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
     __shared__ __align__(8) uint64_t bar_tab[kMmaMaxSlots], bar_seed[kMmaMaxSlots], bar_done[kMmaMaxSlots];
     __shared__ double2 trig64[64];  // (cos, sin)(2 pi j / 64)
 
+    // Warps 0-3 (the first warpgroup) are the seed warps, warps 4-11 the MMA warps `wid` = 0-7: the warp
+    // scheduler favours the oldest (lowest-numbered) of the warps that compete for the FP64 pipe, and the
+    // seed warps' few instructions must not queue behind the two MMA warps of their sub-partition.
+#ifdef FREDEC_EXP_SEED_LAST  // measurement build: the seed warps are the last warpgroup
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const bool seed_warp = wid >= kNW;
+    const int pw = wid - kNW;
+#else
+    const int tid = threadIdx.x, lane = tid & 31, wid = (tid >> 5) - kSeedWarps;
+    const bool seed_warp = wid < 0;
+    const int pw = wid + kSeedWarps;
+#endif
     const int KS = p.TI / 4;  // groups of 4 observations per slot
     const int NS = p.NS;
     const size_t tab_bytes = (size_t)KS * GROUP * 8;
@@ -658,10 +673,9 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
     Cursor c;
     c.init(p, ntiles, CAP);
 
-    if (wid >= kNW) {
+    if (seed_warp) {
         // ================= seed warps: table staging (a4) + seeds (a5) =====================
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(ScanRegs<H, NOCT, NB>::kSeed));
-        const int pw = wid - kNW;
         // lane = (j, mp, k): group pw + 4 j of the slot, observation k of it, runs mp and mp + 4 of each
         // unit.  One exact evaluation per lane and step serves two runs (the second by a rotation).
         const int k = lane & 3, mp = (lane >> 2) & 3, ks = pw + kSeedWarps * (lane >> 4);
@@ -685,13 +699,19 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
             c.advance(ntiles, U, CAP);
             if (c.valid) fetch(c);
             if (!first_lap) mbar_wait(&bar_done[slot], par ^ 1u);
-            unsigned char* base = smem_raw + slot * slot_bytes;
+            // ring layout: the NS table tiles, then the NS seed blocks (consecutive slots adjacent)
+            unsigned char* tab_dst = smem_raw + slot * tab_bytes;
+            unsigned char* seed_dst = smem_raw + NS * tab_bytes + slot * (slot_bytes - tab_bytes);
             if (pw == 0 && lane == 0) {
                 const uint32_t bytes = (uint32_t)ngrp * GROUP * 8u;
                 mbar_expect_tx(&bar_tab[slot], bytes);
-                bulk_g2s(base, tab_src, bytes, &bar_tab[slot]);
+                bulk_g2s(tab_dst, tab_src, bytes, &bar_tab[slot]);
             }
+#ifdef FREDEC_EXP_STUB_SEEDS  // measurement build (wrong results): the seed warps stage the table and arrive
+            if (false) {
+#else
             if (ks < ngrp) {
+#endif
                 // centre of run mp of the round's first unit: f_c = f0 + (run R + H - 1/2) df   (S1)
                 const double kc = (double)((u0 * 8 + mp) * R + H) - 0.5;
                 const double fc = fma(kc, p.df, p.f0);
@@ -704,7 +724,7 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
                 double ca1 = ca0, sa1 = sa0, cb1 = cb0, sb1 = sb0;
                 rotate(ca1, sa1, r.cu, r.su);
                 rotate(cb1, sb1, r.cu, r.su);
-                double2* da = reinterpret_cast<double2*>(base + tab_bytes) + (size_t)ks * CAP * 32 + mp * 4 + k;
+                double2* da = reinterpret_cast<double2*>(seed_dst) + (size_t)ks * CAP * 32 + mp * 4 + k;
                 double2* db = da + 16;  // run mp + 4
                 da[0] = make_double2(ca0, sa0);
                 db[0] = make_double2(cb0, sb0);
