@@ -11,15 +11,16 @@
 // Orthogonalisation = Cholesky QR applied twice.  One pass: the whole weighted Gram matrix of
 // (phi_0 .. phi_{d-1}, x) in ONE sweep over the observations (register tiles of 4 x 4 entries per
 // warp), Cholesky G = L L^T in shared memory with x carried as the last row (that row
-// becomes a = L^{-1} g), then psi = L^{-1} phi and x' = x - sum_j a_j psi_j by one forward
-// substitution per observation.  The first pass leaves an orthogonality error of eps x cond(G); the
+// becomes a = L^{-1} g; one barrier and one reciprocal square root per column), then psi = L^{-1} phi
+// and x' = x - sum_j a_j psi_j by one forward substitution per observation.  The first pass leaves an orthogonality error of eps x cond(G); the
 // second pass, on the already nearly orthonormal functions, removes it ("twice is enough").  This
 // is O(1) sweeps over the data where Gram-Schmidt needs O(d^2) dependent reductions.
 //
-// A series is shared by the C CTAs of a thread-block cluster (C = 1 for short series): each CTA
-// owns a contiguous slice of the observations, the partial Gram matrices (and the scalars of a1)
+// A series is shared by the C CTAs of a thread-block cluster (about 1000 observations per CTA, C <= 8;
+// C = 1 when there are many series): each CTA owns a contiguous slice of the observations, the partial Gram matrices (and the scalars of a1)
 // are added over the cluster through distributed shared memory in rank order, and every CTA then
 // factors the same matrix.  All orders are fixed: results are bitwise reproducible.
+#include <cstdio>
 #include <cooperative_groups.h>
 
 #include "prep_kernel.cuh"
@@ -30,11 +31,12 @@ namespace fredec {
 
 namespace {
 
-constexpr int kPrepThreads = 256;
+constexpr int kPrepThreads = 512;  // at most (one long series); 256 when there are many series
 constexpr int kPrepWarps = kPrepThreads / 32;
 constexpr int kPrepMaxCluster = 8;
 constexpr int kGramTile = 4;       // a warp accumulates a 4 x 4 block of Gram entries
 constexpr int kGramMinSplit = 64;  // observations per warp at least, when a tile's sweep is split between warps
+constexpr int kPrepSliceTarget = 1024;  // observations per CTA aimed at when one series is spread over a cluster
 
 // Shared-memory layout of the prep kernel (doubles), M = d + 1 columns (the base functions and x).
 // `stage` holds the CTA's slice of (w, phi_0 .. phi_{d-1}, x), d + 2 rows of `slice` observations, when it
@@ -42,7 +44,7 @@ constexpr int kGramMinSplit = 64;  // observations per warp at least, when a til
 struct PrepSmem {
     int M, LD, tiles, splits;
     int64_t slice;  // observations per staged row (0: not staged, the passes run on global memory)
-    size_t part, gram, chol, diag0, scal, stage, total;  // offsets in doubles; total in bytes
+    size_t part, gram, chol, fact, diag0, scal, stage, total;  // offsets in doubles; total in bytes
 };
 __host__ __device__ inline PrepSmem prep_smem(int d, int splits, int64_t slice)
 {
@@ -56,41 +58,39 @@ __host__ __device__ inline PrepSmem prep_smem(int d, int splits, int64_t slice)
     size_t o = 0;
     L.part = o;  o += (size_t)splits * L.tiles * 16;   // per (split, tile): a 4 x 4 block
     L.gram = o;  o += (size_t)L.M * L.LD;              // this CTA's partial Gram matrix (read by the cluster)
-    L.chol = o;  o += (size_t)L.M * L.LD;              // the cluster's Gram matrix, factored in place
-    L.diag0 = o; o += L.M;
-    L.scal = o;  o += 16;
+    L.chol = o;  o += (size_t)L.M * L.LD;              // the cluster's Gram matrix, eliminated in place
+    L.fact = o;  o += (size_t)L.M * L.LD;              // its Cholesky factor (row d: a = L^{-1} g)
+    L.diag0 = o; o += 2 * L.M;                         // original diagonal, then 1 / L[j][j]
+    L.scal = o;  o += 16 + 4 * kPrepWarps;
     L.stage = o; o += (size_t)(d + 2) * slice;
     L.total = o * sizeof(double);
     return L;
 }
 
-// Fixed-order block sum, result broadcast to all threads.  `red` = 32 doubles of smem.
-__device__ double block_sum(double v, double* red)
+// Fixed-order block reductions, results broadcast to all threads: v[0], v[1] are summed, v[2], v[3]
+// minimised.  `red` = 4 * kPrepWarps doubles of smem.  One barrier pair for the four of them.
+__device__ void block_reduce4(double v[4], double* red)
 {
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    for (int o = 16; o > 0; o >>= 1) {
+        v[0] += __shfl_xor_sync(0xffffffffu, v[0], o);
+        v[1] += __shfl_xor_sync(0xffffffffu, v[1], o);
+        v[2] = fmin(v[2], __shfl_xor_sync(0xffffffffu, v[2], o));
+        v[3] = fmin(v[3], __shfl_xor_sync(0xffffffffu, v[3], o));
+    }
     __syncthreads();  // protect `red` from the previous call's readers
-    if (lane == 0) red[wid] = v;
+    if (lane == 0)
+        for (int k = 0; k < 4; ++k) red[k * kPrepWarps + wid] = v[k];
     __syncthreads();
-    double r = (lane < kPrepWarps) ? red[lane] : 0.0;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) r += __shfl_xor_sync(0xffffffffu, r, o);
-    return r;
-}
-
-__device__ double block_min(double v, double* red)
-{
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
-    __syncthreads();
-    if (lane == 0) red[wid] = v;
-    __syncthreads();
-    double r = (lane < kPrepWarps) ? red[lane] : v;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) r = fmin(r, __shfl_xor_sync(0xffffffffu, r, o));
-    return r;
+    v[0] = v[1] = 0.0;
+    v[2] = v[3] = INFINITY;
+    for (int q = 0; q < (int)(blockDim.x >> 5); ++q) {  // warp order: the same sum in every thread
+        v[0] += red[q];
+        v[1] += red[kPrepWarps + q];
+        v[2] = fmin(v[2], red[2 * kPrepWarps + q]);
+        v[3] = fmin(v[3], red[3 * kPrepWarps + q]);
+    }
 }
 
 // The CTA's view of its slice: rows (w, columns 0 .. d-1, x) with a common stride, in shared memory
@@ -112,7 +112,7 @@ __device__ void gram_partial(const PrepSmem& L, double* sm, const Rows& R, int d
     const int M = L.M;
     double* part = sm + L.part;
     const int64_t per = (R.n + L.splits - 1) / L.splits;
-    for (int item = wid; item < L.tiles * L.splits; item += kPrepWarps) {
+    for (int item = wid; item < L.tiles * L.splits; item += (blockDim.x >> 5)) {
         const int tile = item % L.tiles, split = item / L.tiles;
         int ta = 0;
         while ((ta + 1) * (ta + 2) / 2 <= tile) ++ta;  // tile = ta (ta + 1) / 2 + tb, tb <= ta
@@ -158,7 +158,7 @@ __device__ void gram_partial(const PrepSmem& L, double* sm, const Rows& R, int d
     }
     __syncthreads();
     double* gram = sm + L.gram;
-    for (int e = threadIdx.x; e < L.tiles * 16; e += kPrepThreads) {
+    for (int e = threadIdx.x; e < L.tiles * 16; e += blockDim.x) {
         const int tile = e / 16, j = (e % 16) / kGramTile, k = e % kGramTile;
         int ta = 0;
         while ((ta + 1) * (ta + 2) / 2 <= tile) ++ta;
@@ -186,7 +186,7 @@ __device__ void gram_cluster_sum(const PrepSmem& L, double* sm, cg::cluster_grou
     cluster_or_cta_sync(cluster, C);  // every CTA's partial matrix is written
     const int M = L.M;
     double* chol = sm + L.chol;
-    for (int e = threadIdx.x; e < M * M; e += kPrepThreads) {
+    for (int e = threadIdx.x; e < M * M; e += blockDim.x) {
         const int a = e / M, b = e % M;
         if (b > a) continue;
         double v = 0.0;
@@ -197,14 +197,17 @@ __device__ void gram_cluster_sum(const PrepSmem& L, double* sm, cg::cluster_grou
     cluster_or_cta_sync(cluster, C);  // all remote reads done before anyone overwrites its partial matrix
 }
 
-// In-place Cholesky of the leading d x d block of chol (lower triangle) with row d (the column x) carried
-// along as a right-hand side: afterwards chol[i][j] = L[i][j], chol[d][j] = a_j = (L^{-1} g)_j,
-// and diag0[j] = 1 / L[j][j].  Returns false when a pivot^2 <= tau x its original diagonal (dependent base
-// functions, S6b).
+// Cholesky of the leading d x d block of chol (lower triangle) with row d (the column x) carried along as
+// a right-hand side.  chol is eliminated in place with UNSCALED columns (so a column is only
+// read while its trailing block is updated: one barrier per column); the factor goes to fact:
+// fact[i][j] = L[i][j], fact[d][j] = a_j = (L^{-1} g)_j, and dinv[j] = 1 / L[j][j].  Returns false when a
+// pivot <= tau x its original diagonal (dependent base functions, S6b).
 __device__ bool chol_with_x(const PrepSmem& L, double* sm, int d, double tau, int* flag)
 {
     double* S = sm + L.chol;
-    double* diag0 = sm + L.diag0;
+    double* F = sm + L.fact;
+    const double* diag0 = sm + L.diag0;
+    double* dinv = sm + L.diag0 + L.M;
     const int LD = L.LD, tid = threadIdx.x;
     if (tid == 0) *flag = 0;
     __syncthreads();
@@ -214,15 +217,13 @@ __device__ bool chol_with_x(const PrepSmem& L, double* sm, int d, double tau, in
             if (tid == 0) *flag = 1;
             break;
         }
-        const double ljj = sqrt(piv), inv = 1.0 / ljj;
-        __syncthreads();
-        for (int i = j + tid; i <= d; i += kPrepThreads) S[i * LD + j] = i == j ? ljj : S[i * LD + j] * inv;
-        if (tid == 0) diag0[j] = inv;  // the original diagonal of column j is not needed again
-        __syncthreads();
+        const double inv = rsqrt(piv), ljj = piv * inv, inv2 = inv * inv;  // one reciprocal square root per column
+        for (int i = j + tid; i <= d; i += blockDim.x) F[i * LD + j] = i == j ? ljj : S[i * LD + j] * inv;
+        if (tid == 0) dinv[j] = inv;
         const int rows = d - j;  // rows j+1 .. d, columns j+1 .. min(row, d-1)
-        for (int e = tid; e < rows * rows; e += kPrepThreads) {
+        for (int e = tid; e < rows * rows; e += blockDim.x) {
             const int i = j + 1 + e / rows, k = j + 1 + e % rows;
-            if (k <= i && k < d) S[i * LD + k] = fma(-S[i * LD + j], S[k * LD + j], S[i * LD + k]);
+            if (k <= i && k < d) S[i * LD + k] = fma(-(S[i * LD + j] * inv2), S[k * LD + j], S[i * LD + k]);
         }
         __syncthreads();
     }
@@ -233,31 +234,47 @@ __device__ bool chol_with_x(const PrepSmem& L, double* sm, int d, double tau, in
 // psi_j(i) = (phi_j(i) - sum_{m<j} L[j][m] psi_m(i)) / L[j][j],  x'(i) = x(i) - sum_j a_j psi_j(i), one
 // thread per observation of the slice; `src` columns (stride src_stride) are read, R.col / R.x written
 // (they may be the same memory: a thread touches its own observation only, and reads back its own writes).
+// The inner sums run on two accumulators with 32-bit offsets: the chain per observation is d sums long,
+// not d^2 / 2 terms.
 __device__ void apply_factor(const PrepSmem& L, double* sm, int d, const double* src, int64_t src_stride,
                              const double* xsrc, const Rows& R)
 {
-    const double* S = sm + L.chol;
-    const double* inv = sm + L.diag0;
-    const int LD = L.LD;
-    for (int64_t i = threadIdx.x; i < R.n; i += kPrepThreads) {
+    const double* F = sm + L.fact;
+    const double* dinv = sm + L.diag0 + L.M;
+    const int LD = L.LD, n = (int)R.n;
+    const bool narrow = R.stride * (int64_t)d < (int64_t)1 << 30;  // offsets fit 32 bits (always, when staged)
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
         double xv = xsrc[i];
+        double* out = R.col + i;
         for (int j = 0; j < d; ++j) {
-            double v = src[(int64_t)j * src_stride + i];
-            const double* row = S + j * LD;
-            for (int m = 0; m < j; ++m) v = fma(-row[m], R.col[(int64_t)m * R.stride + i], v);
-            v *= inv[j];
-            R.col[(int64_t)j * R.stride + i] = v;
-            xv = fma(-S[d * LD + j], v, xv);
+            const double* row = F + j * LD;
+            double s0 = 0.0, s1 = 0.0;
+            if (narrow) {
+                const int st = (int)R.stride;
+                int m = 0;
+                for (; m + 1 < j; m += 2) {
+                    s0 = fma(row[m], out[m * st], s0);
+                    s1 = fma(row[m + 1], out[(m + 1) * st], s1);
+                }
+                if (m < j) s0 = fma(row[m], out[m * st], s0);
+            } else {
+                for (int m = 0; m < j; ++m) s0 = fma(row[m], out[(int64_t)m * R.stride], s0);
+            }
+            const double v = (src[(int64_t)j * src_stride + i] - (s0 + s1)) * dinv[j];
+            out[(int64_t)j * R.stride] = v;
+            xv = fma(-F[d * LD + j], v, xv);
         }
         R.x[i] = xv;
     }
     __syncthreads();
 }
 
+// STAGED: the slice lives in shared memory (the pointers of `Rows` then derive from `sm` alone, so that the
+// compiler addresses them as shared memory instead of through generic loads).
+template <bool STAGED>
 __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p, int splits, int64_t slice)
 {
     extern __shared__ __align__(16) double sm[];
-    __shared__ double red[32];
     __shared__ int flag;
     cg::cluster_group cluster = cg::this_cluster();
     const int C = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
@@ -273,17 +290,40 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p, int sp
     double* xt = p.xt + b * N + i0;                 // [N]
     SeriesInfo* info = p.info + b;
     double* scal = sm + L.scal;
-    const bool staged = slice > 0;
+    double* red = scal + 16;
+    constexpr bool staged = STAGED;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     Rows R;
     R.n = i1 - i0;
-    R.stride = staged ? slice : N;
-    R.w = staged ? sm + L.stage : w;
-    R.col = staged ? sm + L.stage + slice : psi;
-    R.x = staged ? sm + L.stage + (d + 1) * slice : xt;
+    if constexpr (STAGED) {
+        R.stride = slice;
+        R.w = sm + L.stage;
+        R.col = sm + L.stage + slice;
+        R.x = sm + L.stage + (d + 1) * slice;
+    } else {
+        R.stride = N;
+        R.w = w;
+        R.col = psi;
+        R.x = xt;
+    }
 
+#ifdef FREDEC_EXP_PREP_TRACE  // measurement build: cycles per phase of CTA 0, printed at the end
+    long long tr[16];
+    int ntr = 0;
+#define FREDEC_TR()             \
+    do {                        \
+        __syncthreads();        \
+        tr[ntr++] = clock64();  \
+    } while (0)
+#else
+#define FREDEC_TR() \
+    do {            \
+    } while (0)
+#endif
+    FREDEC_TR();
     // ---- a1: validate, W = <1>, time origin; the slice goes to shared memory when it fits -----------
     double bad = 0.0, wsum = 0.0, tmin = INFINITY, tmax = -INFINITY;
-    for (int64_t i = threadIdx.x; i < R.n; i += kPrepThreads) {
+    for (int64_t i = threadIdx.x; i < R.n; i += blockDim.x) {
         const double ti = t[i], xi = x[i], wi = w[i];
         if (!isfinite(ti) || !isfinite(xi) || !isfinite(wi) || wi < 0.0) bad = 1.0;
         wsum += wi;
@@ -294,22 +334,26 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p, int sp
             R.x[i] = xi;
         }
     }
-    // the base functions as one flat sweep (independent loads, whole rows back to back)
-    for (int64_t e = threadIdx.x; e < (int64_t)d * R.n; e += kPrepThreads) {
-        const int64_t j = e / R.n, i = e - j * R.n;
-        const double v = base[j * N + i];
-        if (!isfinite(v)) bad = 1.0;
-        if (staged) R.col[j * slice + i] = v;
+    // the base functions: a warp per row, the lanes along it (independent coalesced loads)
+    for (int j = wid; j < d; j += (blockDim.x >> 5)) {
+        const double* src = base + (int64_t)j * N;
+        double* dst = staged ? R.col + (int64_t)j * slice : nullptr;
+        for (int64_t i = lane; i < R.n; i += 32) {
+            const double v = src[i];
+            if (!isfinite(v)) bad = 1.0;
+            if (staged) dst[i] = v;
+        }
     }
-    bad = block_sum(bad, red);
-    wsum = block_sum(wsum, red);
-    tmin = block_min(tmin, red);
-    tmax = -block_min(-tmax, red);
-    if (threadIdx.x == 0) {
-        scal[0] = bad;
-        scal[1] = wsum;
-        scal[2] = tmin;
-        scal[3] = tmax;
+    FREDEC_TR();
+    {
+        double v4[4] = {bad, wsum, tmin, -tmax};
+        block_reduce4(v4, red);
+        if (threadIdx.x == 0) {
+            scal[0] = v4[0];
+            scal[1] = v4[1];
+            scal[2] = v4[2];
+            scal[3] = -v4[3];
+        }
     }
     cluster_or_cta_sync(cluster, C);
     double W = 0.0;
@@ -323,6 +367,7 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p, int sp
         tmin = fmin(tmin, rs[2]);
         tmax = fmax(tmax, rs[3]);
     }
+    FREDEC_TR();
     int status = 0;
     if (bad != 0.0 || !(W > 0.0) || !isfinite(W)) status = -2;  // FREDEC_EDATA
     const double t_mid = 0.5 * (tmin + tmax);
@@ -333,34 +378,43 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p, int sp
     for (int pass = 0; pass < 2; ++pass) {
         // not staged: the first pass reads the caller's base functions and x, and writes the workspace
         Rows G = R;
-        if (!staged && pass == 0) {
-            G.col = const_cast<double*>(base);
-            G.x = const_cast<double*>(x);
+        if constexpr (!STAGED) {
+            if (pass == 0) {
+                G.col = const_cast<double*>(base);
+                G.x = const_cast<double*>(x);
+            }
         }
         gram_partial(L, sm, G, d);
+        FREDEC_TR();
         gram_cluster_sum(L, sm, cluster, C);
+        FREDEC_TR();
         // pass 0 decides whether the base functions are dependent (S6b); pass 1 factors a matrix
         // that is the identity up to the first pass's orthogonality error
         const bool ok = chol_with_x(L, sm, d, pass == 0 ? kTauBase : 0.0, &flag);
         if (!ok && status == 0) status = -3;  // FREDEC_ESINGULAR (the same decision in every CTA)
+        FREDEC_TR();
         if (ok) apply_factor(L, sm, d, G.col, G.stride, G.x, R);
+        FREDEC_TR();
     }
     double chi2 = 0.0;
-    for (int64_t i = threadIdx.x; i < R.n; i += kPrepThreads) chi2 = fma(R.w[i] * R.x[i], R.x[i], chi2);
-    chi2 = block_sum(chi2, red);
-    if (staged) {  // results to the workspace: whole rows, coalesced
-        for (int64_t e = threadIdx.x; e < (int64_t)d * R.n; e += kPrepThreads) {
-            const int64_t j = e / R.n, i = e - j * R.n;
-            psi[j * N + i] = R.col[j * slice + i];
-        }
-        for (int64_t i = threadIdx.x; i < R.n; i += kPrepThreads) xt[i] = R.x[i];
+    for (int64_t i = threadIdx.x; i < R.n; i += blockDim.x) chi2 = fma(R.w[i] * R.x[i], R.x[i], chi2);
+    {
+        double v4[4] = {chi2, 0.0, 0.0, 0.0};
+        block_reduce4(v4, red);
+        if (threadIdx.x == 0) scal[4] = v4[0];
     }
-    cluster_or_cta_sync(cluster, C);  // the a1 scalars have been read by every CTA
-    if (threadIdx.x == 0) scal[0] = chi2;
+    if (staged) {  // results to the workspace: whole rows, coalesced
+        for (int j = wid; j < d; j += (blockDim.x >> 5)) {
+            const double* src = R.col + (int64_t)j * slice;
+            double* dst = psi + (int64_t)j * N;
+            for (int64_t i = lane; i < R.n; i += 32) dst[i] = src[i];
+        }
+        for (int64_t i = threadIdx.x; i < R.n; i += blockDim.x) xt[i] = R.x[i];
+    }
     cluster_or_cta_sync(cluster, C);
     if (rank == 0 && threadIdx.x == 0) {
         double total = 0.0;
-        for (int r = 0; r < C; ++r) total += cluster.map_shared_rank(scal, r)[0];
+        for (int r = 0; r < C; ++r) total += cluster.map_shared_rank(scal, r)[4];
         info->W = W;
         info->chi2_base = status == 0 ? total : 0.0;
         info->t_mid = t_mid;
@@ -368,6 +422,14 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p, int sp
         info->pad = 0;
     }
     cluster_or_cta_sync(cluster, C);  // no CTA exits while its shared memory may still be read
+#ifdef FREDEC_EXP_PREP_TRACE
+    FREDEC_TR();
+    if (threadIdx.x == 0 && blockIdx.x == 0 && blockIdx.y == 0) {
+        printf("prep trace N=%lld d=%d C=%d (load, reduce, [gram, sum, chol, apply] x 2, rest):", (long long)N, d, C);
+        for (int i = 1; i < ntr; ++i) printf(" %lld", tr[i] - tr[i - 1]);
+        printf(" total %lld\n", tr[ntr - 1] - tr[0]);
+    }
+#endif
 }
 
 // ---- a3: per-observation table and seed records --------------------------
@@ -448,22 +510,25 @@ cudaError_t launch_prep(const PrepParams& p, int64_t B, cudaStream_t stream)
     int C = 1;
     auto fits = [&](int c) { return fixed + (size_t)(p.d + 2) * ((p.N + c - 1) / c) * 8 <= kSmemMax; };
     if (B <= 64)
-        while (C < kPrepMaxCluster && !fits(C)) C *= 2;
+        while (C < kPrepMaxCluster && (!fits(C) || (p.N + C - 1) / C > kPrepSliceTarget)) C *= 2;
     const int64_t per_cta = (p.N + C - 1) / C;
     const int64_t slice = fits(C) ? per_cta : 0;
-    int splits = kPrepWarps / prep_smem(p.d, 1, 0).tiles;
+    const int threads = B <= 64 ? kPrepThreads : 256;  // many series: more CTAs per SM instead
+    int splits = (threads / 32) / prep_smem(p.d, 1, 0).tiles;
     if (splits > (int)(per_cta / kGramMinSplit)) splits = (int)(per_cta / kGramMinSplit);
     if (splits < 1) splits = 1;
     const PrepSmem L = prep_smem(p.d, splits, slice);
-    static size_t attr_smem = 0;
-    if (L.total > attr_smem) {
-        cudaError_t e = cudaFuncSetAttribute(prep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total);
+    static size_t attr_smem[2] = {0, 0};
+    const int st = slice > 0 ? 1 : 0;
+    if (L.total > attr_smem[st]) {
+        cudaError_t e = st ? cudaFuncSetAttribute(prep_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total)
+                           : cudaFuncSetAttribute(prep_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.total);
         if (e != cudaSuccess) return e;
-        attr_smem = L.total;
+        attr_smem[st] = L.total;
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)C, (unsigned)B, 1);
-    cfg.blockDim = dim3(kPrepThreads, 1, 1);
+    cfg.blockDim = dim3(threads, 1, 1);
     cfg.dynamicSmemBytes = L.total;
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
@@ -473,7 +538,8 @@ cudaError_t launch_prep(const PrepParams& p, int64_t B, cudaStream_t stream)
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, prep_kernel, p, splits, slice);
+    return st ? cudaLaunchKernelEx(&cfg, prep_kernel<true>, p, splits, slice)
+              : cudaLaunchKernelEx(&cfg, prep_kernel<false>, p, splits, slice);
 }
 
 }  // namespace fredec
