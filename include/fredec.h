@@ -114,8 +114,12 @@ int fredec_topk_batched(const double* z, int64_t B, int64_t K, int32_t k, int64_
 /*
  * fredec_scan_topk -- the whole hot path in one call: fredec_scan followed by fredec_topk on
  * the periodogram while it is still in device memory (one phase-1 iteration of PAPER.md:201).
- * z_out may be NULL when only the peaks are wanted (the periodogram then stays in a
- * library-owned device buffer and is not copied out).  Other arguments as above.
+ * z_out may be NULL when only the peaks are wanted.  Then, for d <= 9 and k <= 32, NO periodogram is
+ * written anywhere: the peak test runs in the scan kernel's epilogue on the values it has just solved
+ * for (per-warp sorted lists plus one edge record per tile of frequencies, merged by a second small
+ * kernel), so B x K x 8 bytes of device memory and their traffic are not needed; the indices are the
+ * same, bit for bit, as with a periodogram.  For larger d or k the periodogram goes to a
+ * library-owned device buffer instead and is not copied out.  Other arguments as above.
  * Returns the number of peaks written (single series) / FREDEC_OK (batched), or an error.
  */
 int fredec_scan_topk(const double* t, const double* x, const double* w, int64_t N,

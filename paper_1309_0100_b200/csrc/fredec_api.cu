@@ -81,6 +81,7 @@ struct State {
     cudaStream_t stream = nullptr;
     cudaEvent_t ev[kNumEvents] = {};
     DevBuf in_t, in_x, in_w, in_base, in_z, out_z, out_idx, out_chi2;
+    DevBuf fz, fi, fedge, fthr;  // fused peak extraction: lists, edge records, group thresholds
     DevBuf gram, rf, part, p1_base, p1_freq, p1_z, p1_idx, p1_stats, tab, srec, psi, xt, info, ws, red, part_z, part_i, count, sink;
     HostBuf h_info, h_count, h_flag, h_p1;
     DevBuf flag;
@@ -213,6 +214,8 @@ struct Call {
     int64_t* hidx = nullptr;
     size_t idx_count = 0;
     bool staged_inputs = false;  // an input was a host pointer (copied through library memory)
+    bool fused = false;          // the scan kept per-warp peak lists instead of writing z (fm = merge parameters)
+    FusedMergeParams fm;
 };
 
 int resolve_pending();
@@ -229,8 +232,10 @@ int begin_call()
 }
 
 // orthogonalise (prep kernel), table kernel, MMA scan; inputs already on the device
+// fused_k > 0 (peaks only, z_out == nullptr): a11 runs in the scan's epilogue when the scan is a single pass
+// and k <= kFusedMaxK; no periodogram is written then.
 int enqueue_series_mma(Call& c, const double* dt, const double* dx, const double* dw, const double* dbase, int64_t B,
-                       int64_t N, int32_t d, double f0, double df, int64_t K, double* z_out)
+                       int64_t N, int32_t d, double f0, double df, int64_t K, double* z_out, int32_t fused_k)
 {
     cudaStream_t st = g.stream;
     int rc;
@@ -266,7 +271,11 @@ int enqueue_series_mma(Call& c, const double* dt, const double* dx, const double
     CK(cudaEventRecord(g.ev[2], st));
 
     c.z_count = (size_t)B * K;
-    if (z_out == nullptr) {
+    const bool fused = z_out == nullptr && fused_k > 0 && fused_k <= kFusedMaxK && n_pass == 1;
+    if (fused) {
+        c.dz = nullptr;
+        c.hz = nullptr;
+    } else if (z_out == nullptr) {
         CK(g.out_z.reserve(c.z_count * 8));
         c.dz = g.out_z.as<double>();
         c.hz = nullptr;
@@ -311,6 +320,44 @@ int enqueue_series_mma(Call& c, const double* dt, const double* dx, const double
         CK(g.part.reserve((size_t)2 * sp.grid * cfg.NW * mma_part_doubles(NB) * 8));
         sp.part = g.part.as<double>();
     }
+    sp.fused_k = 0;
+    sp.tail_group0 = 0;
+    sp.list_z = nullptr;
+    sp.list_i = nullptr;
+    sp.edges = nullptr;
+    sp.group_thr = nullptr;
+    if (fused) {
+        // one list group per (series, CTA) pair -- group = series + CTA -- and one per left-over round
+        const size_t groups = (size_t)B + sp.grid + sp.Rt;
+        const size_t entries = groups * cfg.NW * fused_k;
+        CK(g.fz.reserve(entries * 8));
+        CK(g.fi.reserve(entries * 8));
+        CK(g.fedge.reserve((size_t)B * U * 4 * 8));
+        CK(g.fthr.reserve(groups * 8));
+        CK(cudaMemsetAsync(g.fi.p, 0xFF, entries * 8, st));  // every entry empty
+        CK(cudaMemsetAsync(g.fthr.p, 0, groups * 8, st));    // no threshold yet
+        sp.group_thr = g.fthr.as<unsigned long long>();
+        sp.fused_k = fused_k;
+        sp.tail_group0 = (int)(B + sp.grid);
+        sp.list_z = g.fz.as<double>();
+        sp.list_i = g.fi.as<int64_t>();
+        sp.edges = g.fedge.as<double>();
+        c.fused = true;
+        c.fm.list_z = sp.list_z;
+        c.fm.list_i = sp.list_i;
+        c.fm.edges = sp.edges;
+        c.fm.info = sp.info;
+        c.fm.K = K;
+        c.fm.U = U;
+        c.fm.T = sp.T;
+        c.fm.unit_points = 8 * R;
+        c.fm.k = fused_k;
+        c.fm.nw = cfg.NW;
+        c.fm.grid = sp.grid;
+        c.fm.shared = sp.shared;
+        c.fm.Rt = sp.Rt;
+        c.fm.tail_group0 = sp.tail_group0;
+    }
     for (int pass = 0; pass < n_pass; ++pass) {
         sp.pass = pass;
         CK(launch_mma_scan(NB, sp, st));
@@ -326,7 +373,7 @@ int enqueue_series_mma(Call& c, const double* dt, const double* dx, const double
 // device pointer, or nullptr (library-owned device buffer, e.g. when only peaks are wanted).
 int enqueue_series(Call& c, const double* t, const double* x, const double* w, int64_t B, int64_t N,
                    const double* base_funcs, int32_t d, double f0, double df, int64_t K, double* z_out,
-                   bool with_scan)
+                   bool with_scan, int32_t fused_k = 0)
 {
     cudaStream_t st = g.stream;
     int rc;
@@ -338,7 +385,7 @@ int enqueue_series(Call& c, const double* t, const double* x, const double* w, i
     if ((rc = stage_in(base_funcs, BN * d, g.in_base, &dbase))) return rc;
     c.staged_inputs = dt != t || dx != x || dw != w || dbase != base_funcs;
 
-    if (with_scan) return enqueue_series_mma(c, dt, dx, dw, dbase, B, N, d, f0, df, K, z_out);
+    if (with_scan) return enqueue_series_mma(c, dt, dx, dw, dbase, B, N, d, f0, df, K, z_out, fused_k);
 
     // base fit only (chi2_base): the prep kernel alone
     CK(g.psi.reserve(BN * (size_t)(d > 0 ? d : 1) * 8));
@@ -386,6 +433,25 @@ int enqueue_topk(Call& c, const double* dz, int64_t B, int64_t K, int32_t k, int
     g.launches += nl;
     CK(cudaEventRecord(g.ev[5], st));
     c.B = B;
+    c.has_topk = true;
+    return FREDEC_OK;
+}
+
+// second stage of the fused peak extraction: merges the scan's lists into idx_out
+int enqueue_fused_merge(Call& c, int64_t B, int32_t k, int64_t* idx_out)
+{
+    cudaStream_t st = g.stream;
+    int rc;
+    c.idx_count = (size_t)B * k;
+    if ((rc = stage_out(idx_out, c.idx_count, g.out_idx, &c.didx, &c.hidx))) return rc;
+    CK(g.count.reserve((size_t)B * sizeof(int)));
+    CK(g.h_count.reserve((size_t)B * sizeof(int)));
+    c.fm.idx_out = c.didx;
+    c.fm.count_out = g.count.as<int>();
+    CK(cudaEventRecord(g.ev[4], st));
+    CK(launch_fused_merge(c.fm, B, st));
+    g.launches += 1;
+    CK(cudaEventRecord(g.ev[5], st));
     c.has_topk = true;
     return FREDEC_OK;
 }
@@ -468,8 +534,9 @@ int do_scan(const double* t, const double* x, const double* w, int64_t B, int64_
     }
     if ((rc = begin_call())) return rc;
     Call c;
-    if ((rc = enqueue_series(c, t, x, w, B, N, base_funcs, d, f0, df, K, z_out, true))) return rc;
-    if (want_topk && (rc = enqueue_topk(c, c.dz, B, K, k, idx_out))) return rc;
+    if ((rc = enqueue_series(c, t, x, w, B, N, base_funcs, d, f0, df, K, z_out, true, want_topk ? k : 0))) return rc;
+    if (want_topk && (rc = c.fused ? enqueue_fused_merge(c, B, k, idx_out) : enqueue_topk(c, c.dz, B, K, k, idx_out)))
+        return rc;
     int count = 0;
     if ((rc = finish_call(c, &count, defer))) return rc;
     return (want_topk && B == 1) ? count : FREDEC_OK;
@@ -948,7 +1015,7 @@ const char* fredec_bench_fp64_name(int32_t mode)
 
 int fredec_shutdown(void)
 {
-    DevBuf* bufs[] = {&g.in_t, &g.in_x, &g.in_w, &g.in_base, &g.in_z, &g.out_z, &g.out_idx, &g.out_chi2, &g.gram, &g.rf, &g.part, &g.p1_base, &g.p1_freq, &g.p1_z, &g.p1_idx, &g.p1_stats, &g.tab, &g.srec,
+    DevBuf* bufs[] = {&g.fz, &g.fi, &g.fedge, &g.fthr, &g.in_t, &g.in_x, &g.in_w, &g.in_base, &g.in_z, &g.out_z, &g.out_idx, &g.out_chi2, &g.gram, &g.rf, &g.part, &g.p1_base, &g.p1_freq, &g.p1_z, &g.p1_idx, &g.p1_stats, &g.tab, &g.srec,
                       &g.psi,  &g.xt,   &g.info, &g.ws, &g.red,     &g.part_z, &g.part_i, &g.count, &g.sink};
     for (DevBuf* b : bufs) b->release();
     g.h_info.release();

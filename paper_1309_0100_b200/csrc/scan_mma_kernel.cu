@@ -60,6 +60,7 @@
 // (which share the FP64 pipe with the MMAs) is off the MMA warps' critical path.
 // Every accumulation order is fixed, so results are bitwise reproducible run to run.
 #include "scan_mma_kernel.cuh"
+#include "topk_list.cuh"
 
 namespace fredec {
 
@@ -529,20 +530,102 @@ __device__ __forceinline__ double solve_z(double YC, double YS, double CC, doubl
     return z;
 }
 
+// a11 fused into the epilogue: the peaks among the 8R grid points of one unit, held as zu[t] (run position
+// H + 4t + q) and zl[t] (position H - 1 - 4t - q) by thread (run m = lane / 4, q = lane % 4), go to the warp's
+// sorted top-k list of its (series, CTA) pair in global memory; the unit's first and last point, whose outer
+// neighbours belong to other units, go to the unit's edge record instead.  A unit with no value at or above
+// the list's k-th entry costs two shuffles, one vote and two small loads.
+template <int H>
+__device__ __forceinline__ void fused_emit(double (&zu)[H / 4], double (&zl)[H / 4], const MmaScanParams& p, int64_t b,
+                                           int64_t unit, int lane, int64_t group, int w, unsigned long long thr_bits)
+{
+    constexpr int R = 2 * H, NT = H / 4;
+    constexpr unsigned kFull = 0xffffffffu;
+    const int m = lane >> 2, q = lane & 3, quad = lane & ~3;
+    const int64_t k0 = (unit * 8 + m) * R;
+    // points past the end of the grid and NaN count as -infinity (S7)
+    double vmax = -INFINITY;
+#pragma unroll
+    for (int t = 0; t < NT; ++t) {
+        zu[t] = k0 + H + 4 * t + q < p.K ? sanitize(zu[t]) : -INFINITY;
+        zl[t] = k0 + H - 1 - 4 * t - q < p.K ? sanitize(zl[t]) : -INFINITY;
+        vmax = fmax(vmax, fmax(zu[t], zl[t]));
+    }
+    // edge record: the half of the peak test that the unit can decide
+    const double right_of_first = __shfl_sync(kFull, zl[NT - 1], 2);  // run 0, position 1
+    const double left_of_last = __shfl_sync(kFull, zu[NT - 1], 30);   // run 7, position R - 2
+    double2* er = reinterpret_cast<double2*>(p.edges + (b * p.U + unit) * 4);
+    if (lane == 3) __stcg(er, make_double2(zl[NT - 1], zl[NT - 1] >= right_of_first ? 1.0 : 0.0));
+    if (lane == 31) __stcg(er + 1, make_double2(zu[NT - 1], zu[NT - 1] > left_of_last ? 1.0 : 0.0));
+    // nothing at or above the group's threshold (the largest k-th entry of its full lists): no candidate
+    const double group_thr = thr_bits ? __longlong_as_double((long long)thr_bits) : -INFINITY;
+    if (!__any_sync(kFull, vmax >= group_thr)) return;
+    // the warp's list
+    const int k = p.fused_k;
+    double* lz = p.list_z + ((size_t)group * kNW + w) * k;
+    int64_t* li = p.list_i + ((size_t)group * kNW + w) * k;
+    WarpList<1> L;
+    L.init(k, lane);
+    if (lane < k) {
+        const int64_t id = __ldcg(li + lane);
+        if (id >= 0 && id != kEmptyIdx) {
+            L.z[0] = __ldcg(lz + lane);
+            L.id[0] = id;
+        }
+    }
+    L.thr_z = __shfl_sync(kFull, L.z[0], k - 1);
+    L.thr_i = shfl_i64(L.id[0], k - 1);
+    const double next_run_first = __shfl_down_sync(kFull, zl[NT - 1], 4);  // position 0 of run m + 1 (lane q = 3)
+    const double prev_run_last = __shfl_up_sync(kFull, zu[NT - 1], 4);     // position R - 1 of run m - 1
+#pragma unroll
+    for (int t = 0; t < NT; ++t) {
+        {  // upper half, position H + 4t + q: left is lane q - 1 | step t - 1 of q = 3 | own zl[0]
+            const double a = __shfl_up_sync(kFull, zu[t], 1), c = __shfl_down_sync(kFull, zu[t], 1);
+            const double a3 = __shfl_sync(kFull, zu[t > 0 ? t - 1 : 0], quad | 3);
+            const double c0 = __shfl_sync(kFull, zu[t < NT - 1 ? t + 1 : t], quad);
+            const double left = q > 0 ? a : (t > 0 ? a3 : zl[0]);
+            const double right = q < 3 ? c : (t < NT - 1 ? c0 : next_run_first);
+            const bool inner = !(t == NT - 1 && lane == 31);  // the unit's last point: edge record
+            L.offer(zu[t], k0 + H + 4 * t + q, inner && zu[t] > left && zu[t] >= right);
+        }
+        {  // lower half, position H - 1 - 4t - q: right is lane q - 1 | step t - 1 of q = 3 | own zu[0]
+            const double c = __shfl_up_sync(kFull, zl[t], 1), a = __shfl_down_sync(kFull, zl[t], 1);
+            const double c3 = __shfl_sync(kFull, zl[t > 0 ? t - 1 : 0], quad | 3);
+            const double a0 = __shfl_sync(kFull, zl[t < NT - 1 ? t + 1 : t], quad);
+            const double right = q > 0 ? c : (t > 0 ? c3 : zu[0]);
+            const double left = q < 3 ? a : (t < NT - 1 ? a0 : prev_run_last);
+            const bool inner = !(t == NT - 1 && lane == 3);  // the unit's first point: edge record
+            L.offer(zl[t], k0 + H - 1 - 4 * t - q, inner && zl[t] > left && zl[t] >= right);
+        }
+    }
+    if (lane < k) {
+        __stcg(lz + lane, L.z[0]);
+        __stcg(li + lane, L.id[0]);
+    }
+    // a full list raises the group's threshold to its k-th entry (z >= 0: the bit patterns order like the values)
+    if (lane == 0 && L.thr_i != kEmptyIdx && L.thr_z > group_thr)
+        atomicMax(p.group_thr + group, (unsigned long long)__double_as_longlong(L.thr_z));
+}
+
 // a9/a10 for the units of one warp after the last tile of a round: this thread holds every sum
 // of 2 * NT frequencies per unit.
-template <int H, int NOCT, int NB>
+// FUSED: nothing is stored; the values of a unit go to fused_emit (a11) with the warp's list (group, w).
+template <int H, int NOCT, int NB, bool FUSED>
 __device__ __forceinline__ void solve_and_store(const Tiles<H, NOCT, NB>& acc, const MmaScanParams& p, int64_t b,
-                                                int64_t unit0, int cnt, int lane)
+                                                int64_t unit0, int cnt, int lane, int64_t group = 0, int w = 0)
 {
     constexpr int R = 2 * H, NT = H / 4, NF = NB + 2;
     const SeriesInfo info = p.info[b];
     const int m = lane >> 2, q = lane & 3;
     const bool last_pass = p.pass + 1 == p.n_pass;
+    if (FUSED && info.status != 0) return;  // no periodogram for this series: no lists, no edge records
+    unsigned long long thr_bits = 0;  // fetched before the solves, used after them
+    if constexpr (FUSED) thr_bits = __ldcg(p.group_thr + group);
 #pragma unroll
     for (int o = 0; o < NOCT; ++o) {
         if (o < cnt) {
             const int64_t k0 = ((unit0 + o) * 8 + m) * R;  // first grid point of the run
+            double zz[2][NT];  // FUSED: z at positions H + 4t + q (sg = 0) and H - 1 - 4t - q (sg = 1)
 #pragma unroll
             for (int t = 0; t < NT; ++t) {
                 const int h = 4 * t + q + 1;
@@ -565,7 +648,9 @@ __device__ __forceinline__ void solve_and_store(const Tiles<H, NOCT, NB>& acc, c
                         Sab = fma(sums[1 + j][0], sums[1 + j][1], Sab);
                         Sbb = fma(sums[1 + j][1], sums[1 + j][1], Sbb);
                     }
-                    if (k < p.K && info.status == 0) {
+                    if constexpr (FUSED) {
+                        zz[sg][t] = solve_z(YC, YS, CC, CS, Saa, Sab, Sbb, info.W);
+                    } else if (k < p.K && info.status == 0) {
                         if (p.n_pass > 1) {  // multi-pass: carry the seven partial sums through global memory
                             double* wsp = p.ws + (b * 7) * p.Kpad + k;
                             if (p.pass > 0) {
@@ -592,6 +677,10 @@ __device__ __forceinline__ void solve_and_store(const Tiles<H, NOCT, NB>& acc, c
                         if (last_pass) p.z[b * p.K + k] = solve_z(YC, YS, CC, CS, Saa, Sab, Sbb, info.W);
                     }
                 }
+            }
+            if constexpr (FUSED) {
+                // (a left-over round of the shared mode can reach past the last unit)
+                if (unit0 + o < p.U) fused_emit<H>(zz[0], zz[1], p, b, unit0 + o, lane, group, w, thr_bits);
             }
         }
     }
@@ -628,7 +717,7 @@ __device__ __forceinline__ void rotate(double& c, double& s, double rc, double r
     s = ns;
 }
 
-template <int H, int NOCT, int NB>
+template <int H, int NOCT, int NB, bool FUSED>
 __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
 {
     constexpr int R = 2 * H, NT = H / 4, NF = NB + 2, GROUP = NF * NT * 32, CAP = kNW * NOCT;
@@ -828,7 +917,7 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
                                 __stcg(dst + ((((o * 2 + x) * NF + f) * NT + t) * 2 + 1) * 32, acc.v[o][x][f][t][1]);
                             }
             } else if (solve) {
-                solve_and_store<H, NOCT, NB>(acc, p, c.b, c.u + role.off, role.cnt, lane);
+                solve_and_store<H, NOCT, NB, FUSED>(acc, p, c.b, c.u + role.off, role.cnt, lane, c.b + blockIdx.x, wid);
             }
             acc.clear();
             c.next_round(U, CAP);
@@ -838,7 +927,7 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
 
 // Shared mode: adds the partial sums of the segments of left-over round blockIdx.x in the order of
 // the CTAs that produced them (fixed: bitwise reproducible), then a9/a10 as in the scan kernel.
-template <int H, int NOCT, int NB>
+template <int H, int NOCT, int NB, bool FUSED>
 __global__ void __launch_bounds__(kNW * 32) tail_solve_kernel(MmaScanParams p)
 {
     constexpr int NT = H / 4, NF = NB + 2, CAP = kNW * NOCT, ACCW = NOCT * 2 * NF * NT * 2;
@@ -870,25 +959,26 @@ __global__ void __launch_bounds__(kNW * 32) tail_solve_kernel(MmaScanParams p)
                     }
     }
     const int64_t u = (int64_t)p.grid * p.F * CAP + r * CAP + wid * NOCT;
-    solve_and_store<H, NOCT, NB>(acc, p, 0, u, NOCT, lane);
+    solve_and_store<H, NOCT, NB, FUSED>(acc, p, 0, u, NOCT, lane, p.tail_group0 + r, wid);
 }
 
-template <int H, int NOCT, int NB>
+template <int H, int NOCT, int NB, bool FUSED>
 cudaError_t launch_one(const MmaScanParams& p, cudaStream_t stream)
 {
     const size_t smem = (size_t)p.NS * mma_scan_slot_bytes(NB, p.TI) + kPipePad;
     static size_t attr_smem = 0;
     if (smem > attr_smem) {
-        cudaError_t e = cudaFuncSetAttribute(scan_mma_kernel<H, NOCT, NB>,
+        cudaError_t e = cudaFuncSetAttribute(scan_mma_kernel<H, NOCT, NB, FUSED>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_smem = smem;
     }
     if (p.NS < 2 || p.NS > kMmaMaxSlots || p.TI < 4 || p.TI % 4 || p.TI > 16 * kSeedGroups) return cudaErrorInvalidValue;
-    scan_mma_kernel<H, NOCT, NB><<<p.grid, kThreads, smem, stream>>>(p);
+    if (FUSED && (p.n_pass != 1 || p.fused_k < 1 || p.fused_k > kFusedMaxK)) return cudaErrorInvalidValue;
+    scan_mma_kernel<H, NOCT, NB, FUSED><<<p.grid, kThreads, smem, stream>>>(p);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess || !p.shared || p.Rt == 0) return e;
-    tail_solve_kernel<H, NOCT, NB><<<p.Rt, kNW * 32, 0, stream>>>(p);
+    tail_solve_kernel<H, NOCT, NB, FUSED><<<p.Rt, kNW * 32, 0, stream>>>(p);
     return cudaGetLastError();
 }
 
@@ -930,7 +1020,7 @@ size_t mma_part_doubles(int NB)
 cudaError_t launch_mma_scan(int NB, const MmaScanParams& p, cudaStream_t stream)
 {
 #define X(h, noct, nb) \
-    if (NB == nb) return launch_one<h, noct, nb>(p, stream);
+    if (NB == nb) return p.fused_k > 0 ? launch_one<h, noct, nb, true>(p, stream) : launch_one<h, noct, nb, false>(p, stream);
     FREDEC_MMA_CONFIGS(X)
 #undef X
     return cudaErrorInvalidValue;

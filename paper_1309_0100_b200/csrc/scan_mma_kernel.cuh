@@ -49,7 +49,21 @@ struct MmaScanParams {
     // shared mode (one series, one pass; see Cursor in scan_mma_kernel.cu): F full rounds per CTA, then
     // Rt left-over rounds cut across the observations and finished by the tail-solve kernel
     int shared, F, Rt;
+    // Fused peak extraction (a11 in the epilogue; z == nullptr, one pass): every MMA warp keeps a sorted
+    // top-k list per (series, CTA) pair -- list group = series + CTA, a bijection for contiguous ranges;
+    // the left-over rounds of the shared mode use the groups tail_group0 + round -- and every unit writes
+    // an edge record (its first and last grid point cannot be tested inside the unit).
+    // topk_fused_merge_kernel (topk_kernel.cu) merges the lists and settles the unit boundaries.
+    int fused_k;         // 0: off (z is written); else k <= kFusedMaxK
+    int tail_group0;
+    double* list_z;      // [groups][MMA warps][fused_k]
+    int64_t* list_i;     // same shape; < 0: empty entry (filled with 0xFF bytes before the launch)
+    double* edges;       // [B][U][4]: z_first, first_ok, z_last, last_ok (flags 1.0 / 0.0)
+    // [groups]: bit pattern of the largest k-th entry among the group's full lists (0: none yet; z >= 0, so
+    // the patterns order like the values).  A value below it cannot be among the series' k highest peaks.
+    unsigned long long* group_thr;
 };
+constexpr int kFusedMaxK = 32;  // one list entry per lane
 
 struct MmaScanConfig {
     int H, NOCT, NW;  // half run length, units per MMA warp and round, MMA warps per CTA

@@ -13,6 +13,7 @@
 #include <cmath>
 #include <cstdint>
 #include "topk_kernel.cuh"
+#include "topk_list.cuh"
 
 namespace fredec {
 
@@ -23,103 +24,6 @@ namespace {
 #endif
 constexpr int kTopkThreads = FREDEC_TOPK_THREADS;
 constexpr int kTopkWarps = kTopkThreads / 32;
-constexpr int64_t kEmptyIdx = INT64_MAX;
-
-__device__ __forceinline__ bool beats(double za, int64_t ia, double zb, int64_t ib)
-{
-    return za > zb || (za == zb && ia < ib);
-}
-__device__ __forceinline__ double sanitize(double v) { return (v != v) ? -INFINITY : v; }
-__device__ __forceinline__ int64_t shfl_i64(int64_t v, int src)
-{
-    return (int64_t)__shfl_sync(0xffffffffu, (long long)v, src);
-}
-__device__ __forceinline__ int64_t shfl_up_i64(int64_t v)
-{
-    return (int64_t)__shfl_up_sync(0xffffffffu, (long long)v, 1);
-}
-
-template <int SLOTS>
-struct WarpList {
-    double z[SLOTS];
-    int64_t id[SLOTS];
-    double thr_z;  // the k-th entry (rank k-1), broadcast to all lanes
-    int64_t thr_i;
-    int k, lane;
-
-    __device__ __forceinline__ void init(int k_, int lane_)
-    {
-        k = k_;
-        lane = lane_;
-#pragma unroll
-        for (int s = 0; s < SLOTS; ++s) {
-            z[s] = -INFINITY;
-            id[s] = kEmptyIdx;
-        }
-        thr_z = -INFINITY;
-        thr_i = kEmptyIdx;
-    }
-    // all lanes call with the same candidate
-    __device__ __forceinline__ void insert(double zc, int64_t ic)
-    {
-        if (!beats(zc, ic, thr_z, thr_i)) return;
-        double carry_z = 0.0;  // entry of rank 32*s - 1 (lane 31 of the previous slot)
-        int64_t carry_i = 0;
-        bool carry_b = false;  // does the candidate beat that entry
-#pragma unroll
-        for (int s = 0; s < SLOTS; ++s) {
-            const bool b = beats(zc, ic, z[s], id[s]);
-            double pz = __shfl_up_sync(0xffffffffu, z[s], 1);
-            int64_t pi = shfl_up_i64(id[s]);
-            bool pb = (bool)__shfl_up_sync(0xffffffffu, (int)b, 1);
-            if (lane == 0) {
-                pz = carry_z;
-                pi = carry_i;
-                pb = (s == 0) ? false : carry_b;
-            }
-            carry_z = __shfl_sync(0xffffffffu, z[s], 31);
-            carry_i = shfl_i64(id[s], 31);
-            carry_b = (bool)__shfl_sync(0xffffffffu, (int)b, 31);
-            if (b) {
-                z[s] = pb ? pz : zc;
-                id[s] = pb ? pi : ic;
-            }
-        }
-        const int rk = k - 1;
-        double tz = -INFINITY;
-        int64_t ti = kEmptyIdx;
-#pragma unroll
-        for (int s = 0; s < SLOTS; ++s)
-            if (s == rk / 32) {
-                tz = __shfl_sync(0xffffffffu, z[s], rk % 32);
-                ti = shfl_i64(id[s], rk % 32);
-            }
-        thr_z = tz;
-        thr_i = ti;
-    }
-    // each lane proposes its own candidate (valid or not)
-    __device__ __forceinline__ void offer(double zc, int64_t ic, bool valid)
-    {
-        unsigned m = __ballot_sync(0xffffffffu, valid && beats(zc, ic, thr_z, thr_i));
-        while (m) {
-            const int src = __ffs(m) - 1;
-            m &= m - 1;
-            insert(__shfl_sync(0xffffffffu, zc, src), shfl_i64(ic, src));
-        }
-    }
-    __device__ __forceinline__ void store(double* dz, int64_t* di) const
-    {
-#pragma unroll
-        for (int s = 0; s < SLOTS; ++s) {
-            const int r = s * 32 + lane;
-            if (r < k) {
-                dz[r] = z[s];
-                di[r] = id[s];
-            }
-        }
-    }
-};
-
 // Merge the CTA's warp lists (smem) into warp 0's list; then write either the final indices
 // (last stage) or this CTA's partial list.
 template <int SLOTS>
@@ -248,6 +152,84 @@ __global__ void __launch_bounds__(kTopkThreads) topk_merge_kernel(TopkParams p)
     cta_merge_and_write<SLOTS>(L, p, b, 0, true, sz, si);
 }
 
+// CTA that owns unit g of the scan's contiguous partition [c T / grid, (c + 1) T / grid)
+__device__ __forceinline__ int unit_owner(int64_t g, int64_t T, int grid)
+{
+    int c = (int)(g * grid / T);
+    while (c + 1 < grid && (int64_t)(c + 1) * T / grid <= g) ++c;
+    while (c > 0 && (int64_t)c * T / grid > g) --c;
+    return c;
+}
+
+__global__ void __launch_bounds__(kTopkThreads) topk_fused_merge_kernel(FusedMergeParams p)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double* sz = reinterpret_cast<double*>(smem_raw);
+    int64_t* si = reinterpret_cast<int64_t*>(sz + kTopkWarps * p.k);
+    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t b = blockIdx.x;
+    WarpList<1> L;
+    L.init(p.k, lane);
+    if (p.info[b].status == 0) {
+        // the lists of the groups that hold this series: two ranges [g0, g1) and [h0, h1)
+        int64_t g0, g1, h0 = 0, h1 = 0;
+        if (p.shared) {
+            g0 = 0;
+            g1 = p.grid;
+            h0 = p.tail_group0;
+            h1 = h0 + p.Rt;
+        } else {
+            g0 = b + unit_owner(b * p.U, p.T, p.grid);
+            g1 = b + unit_owner((b + 1) * p.U - 1, p.T, p.grid) + 1;
+        }
+        const int64_t per = (int64_t)p.nw * p.k;
+        const int64_t n1 = (g1 - g0) * per, total = n1 + (h1 - h0) * per;
+        for (int64_t base = (int64_t)wid * 32; base < total; base += kTopkThreads) {
+            const int64_t e = base + lane;
+            bool valid = e < total;
+            double zc = -INFINITY;
+            int64_t ic = kEmptyIdx;
+            if (valid) {
+                const int64_t at = e < n1 ? g0 * per + e : h0 * per + (e - n1);
+                ic = __ldcg(p.list_i + at);
+                valid = ic >= 0 && ic != kEmptyIdx;
+                if (valid) zc = __ldcg(p.list_z + at);
+            }
+            L.offer(zc, ic, valid);
+        }
+        // unit boundaries: the first point of unit u is a peak iff first_ok and z_first > z_last of unit u - 1;
+        // the last point iff last_ok and z_last >= z_first of unit u + 1 (outside the grid: -infinity)
+        const double* ed = p.edges + b * p.U * 4;
+        for (int64_t base = (int64_t)wid * 32; base < p.U; base += kTopkThreads) {
+            const int64_t u = base + lane;
+            bool pf = false, pl = false;
+            double zf = -INFINITY, zl = -INFINITY;
+            if (u < p.U) {
+                const double2 f = __ldcg(reinterpret_cast<const double2*>(ed + u * 4));
+                const double2 l = __ldcg(reinterpret_cast<const double2*>(ed + u * 4 + 2));
+                const double before = u > 0 ? __ldcg(ed + (u - 1) * 4 + 2) : -INFINITY;
+                const double after = u + 1 < p.U ? __ldcg(ed + (u + 1) * 4) : -INFINITY;
+                zf = f.x;
+                zl = l.x;
+                pf = f.y != 0.0 && zf > before;
+                pl = l.y != 0.0 && zl >= after;
+            }
+            L.offer(zf, u * p.unit_points, pf);
+            L.offer(zl, (u + 1) * p.unit_points - 1, pl);
+        }
+    }
+    TopkParams tp;
+    tp.z = nullptr;
+    tp.idx_out = p.idx_out;
+    tp.count_out = p.count_out;
+    tp.part_z = nullptr;
+    tp.part_i = nullptr;
+    tp.K = p.K;
+    tp.k = p.k;
+    tp.nblk = 1;
+    cta_merge_and_write<1>(L, tp, b, 0, true, sz, si);
+}
+
 template <int SLOTS>
 cudaError_t launch_slots(const TopkParams& p, int64_t B, cudaStream_t stream, int* launches)
 {
@@ -269,6 +251,14 @@ cudaError_t launch_slots(const TopkParams& p, int64_t B, cudaStream_t stream, in
 }
 
 }  // namespace
+
+cudaError_t launch_fused_merge(const FusedMergeParams& p, int64_t B, cudaStream_t stream)
+{
+    if (p.k < 1 || p.k > 32) return cudaErrorInvalidValue;
+    const size_t smem = (size_t)kTopkWarps * p.k * 16;
+    topk_fused_merge_kernel<<<(unsigned)B, kTopkThreads, smem, stream>>>(p);
+    return cudaGetLastError();
+}
 
 int topk_pick_nblk(int64_t B, int64_t K, int sm_count)
 {
