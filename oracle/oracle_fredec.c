@@ -299,10 +299,14 @@ int oracle_topk(const double *z, int64_t K, int32_t k, int64_t *idx_out)
     return found;
 }
 
+/* threads a parallel loop can use on this machine: the processors available to the process, capped by
+ * OMP_NUM_THREADS at start-up -- NOT the value of the last oracle_set_threads call */
 int oracle_num_threads(void)
 {
 #ifdef _OPENMP
-    return omp_get_max_threads();
+    static int at_start = 0;
+    if (at_start == 0) at_start = omp_get_max_threads();
+    return at_start < omp_get_num_procs() ? at_start : omp_get_num_procs();
 #else
     return 1;
 #endif

@@ -2,6 +2,8 @@
 against oracle/phase1.py, through the C-ABI binding.  Integer results (grid indices, counts)
 must be identical; floating point within 1e-12 relative (element-wise maps: a handful of
 correctly rounded operations) and 1e-9 relative for statistics derived from a scan."""
+import os
+
 import numpy as np
 import pytest
 
@@ -347,6 +349,7 @@ def test_refine_batched_parity_1000_tuples(fr, p1, oracle_mod):
     fd, ld, _, _ = fr.fredec_refine_batched(*[torch.from_numpy(a).cuda() for a in (t, x, w, pool)], masks[:50],
                                              max_iter=30, tol=tol)
     assert np.array_equal(fd, freqs[:50]) and np.array_equal(ld, l[:50])
+    os.makedirs("gpurun_out", exist_ok=True)
     with open("gpurun_out/refine_batched.txt", "w") as fh:
         tm = fr.fredec_last_timing()
         fh.write(f"tuples=50 kernel_ms={tm['scan_ms']:.3f}\n")
