@@ -45,8 +45,8 @@ ORACLE_SAMPLE_K = 100_000         # grid points of config 4 the CPU legs time pe
 # `ncu --set full` capture summarised in the file named below -- NOT measured in the bench run (ncu
 # cannot run inside it).  Algorithmic bytes: table + seed records + 16 MB z (the periodogram is still
 # in L2 when the kernel ends, so the capture sees less than that).
-SCAN_DRAM_TRAFFIC_BYTES = 12_090_112
-SCAN_DRAM_TRAFFIC_SOURCE = "profiles/r1_scan_mma_kernel_ncu.md (ncu --set full capture; not measured in this run)"
+SCAN_DRAM_TRAFFIC_BYTES = 21_257_472   # 15.93 MB read + 5.33 MB written
+SCAN_DRAM_TRAFFIC_SOURCE = "profiles/r2_scan_cfg4_ncu.md (ncu --set full capture; not measured in this run)"
 
 
 def flops_per_pair(d: int) -> int:

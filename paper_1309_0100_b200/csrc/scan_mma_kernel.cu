@@ -579,6 +579,9 @@ __device__ __forceinline__ void fused_emit(double (&zu)[H / 4], double (&zl)[H /
     const double prev_run_last = __shfl_up_sync(kFull, zu[NT - 1], 4);     // position R - 1 of run m - 1
 #pragma unroll
     for (int t = 0; t < NT; ++t) {
+        // a step none of whose 64 points reaches the list's k-th entry (which rises as the unit is read) needs
+        // no neighbours: almost every step of a unit that got this far
+        if (!__any_sync(kFull, zu[t] >= L.thr_z || zl[t] >= L.thr_z)) continue;
         {  // upper half, position H + 4t + q: left is lane q - 1 | step t - 1 of q = 3 | own zl[0]
             const double a = __shfl_up_sync(kFull, zu[t], 1), c = __shfl_down_sync(kFull, zu[t], 1);
             const double a3 = __shfl_sync(kFull, zu[t > 0 ? t - 1 : 0], quad | 3);
