@@ -271,7 +271,10 @@ __device__ __forceinline__ double twice(double x)
 }
 
 // a6 for one group of 4 observations: A fragments (seeds), B fragments (table), 2 * NF * NT MMAs per unit.
-template <int CNT, int H, int NOCT, int NB>
+// BASE_ONLY (passes after the first of a scan with more than 9 base functions): the y and w/2 families of
+// such a pass have all-zero tables (their sums were formed by the first pass and are carried in the
+// workspace), so their MMAs are left out.
+template <int CNT, int H, int NOCT, int NB, bool BASE_ONLY>
 __device__ __forceinline__ void mma_group(Tiles<H, NOCT, NB>& acc, const double2* tk, const double2* sk)
 {
     constexpr int NT = H / 4, NF = NB + 2;
@@ -287,7 +290,7 @@ __device__ __forceinline__ void mma_group(Tiles<H, NOCT, NB>& acc, const double2
         s2[o] = tc * a[o].y;            // sin 2 phi = 2 cos phi sin phi
     }
 #pragma unroll
-    for (int f = 0; f < NF; ++f) {
+    for (int f = BASE_ONLY ? 1 : 0; f < (BASE_ONLY ? NF - 1 : NF); ++f) {
 #pragma unroll
         for (int tp = 0; tp < NT / 2; ++tp) {
             const double2 b2 = tk[(f * (NT / 2) + tp) * 32];
@@ -455,7 +458,7 @@ __device__ __forceinline__ void round_mma_pipelined(Tiles<H, 1, NB>& acc, RingPo
 // a6 for one round: all tiles of the series, CNT = units this warp owns in the round.  The ring slot
 // changes every KS groups; the next slot's barriers are looked at before the slot's last groups so
 // that the MMA stream continues across slots.
-template <int CNT, int H, int NOCT, int NB>
+template <int CNT, bool BASE_ONLY, int H, int NOCT, int NB>
 __device__ __forceinline__ void round_mma(Tiles<H, NOCT, NB>& acc, RingPos& rp, const unsigned char* smem,
                                           size_t slot_bytes, size_t tab_bytes, int NS, int KS, int64_t G4,
                                           int tile0, int tile1, WarpRole role, int lane, uint64_t* bar_tab,
@@ -485,15 +488,15 @@ __device__ __forceinline__ void round_mma(Tiles<H, NOCT, NB>& acc, RingPos& rp, 
             const int head = ngrp > 2 ? (ngrp - 2) & ~1 : 0;
 #pragma unroll 1
             for (int ks = 0; ks < head; ks += 2) {
-                mma_group<CNT>(acc, tk, sk);
-                mma_group<CNT>(acc, tk + GROUP2, sk + CAP * 32);
+                mma_group<CNT, H, NOCT, NB, BASE_ONLY>(acc, tk, sk);
+                mma_group<CNT, H, NOCT, NB, BASE_ONLY>(acc, tk + GROUP2, sk + CAP * 32);
                 tk += 2 * GROUP2;
                 sk += 2 * CAP * 32;
             }
             rp.ready = mbar_test(&bar_tab[nslot], npar) & mbar_test(&bar_seed[nslot], npar);
 #pragma unroll 1
             for (int ks = head; ks < ngrp; ++ks) {
-                mma_group<CNT>(acc, tk, sk);
+                mma_group<CNT, H, NOCT, NB, BASE_ONLY>(acc, tk, sk);
                 tk += GROUP2;
                 sk += CAP * 32;
             }
@@ -502,7 +505,7 @@ __device__ __forceinline__ void round_mma(Tiles<H, NOCT, NB>& acc, RingPos& rp, 
             rp.ready = false;
 #pragma unroll 1
             for (int ks = role.sp; ks < ngrp; ks += role.S)
-                mma_group<CNT>(acc, tk + (size_t)ks * GROUP2, sk + (size_t)ks * CAP * 32);
+                mma_group<CNT, H, NOCT, NB, BASE_ONLY>(acc, tk + (size_t)ks * GROUP2, sk + (size_t)ks * CAP * 32);
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&bar_done[rp.slot]);
@@ -850,9 +853,13 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
         while (c.valid) {  // one round per iteration
             const WarpRole role = warp_role(c.n, wid);
 #define FREDEC_ROUND(CNT) \
-    round_mma<CNT>(acc, rp, smem_raw, slot_bytes, tab_bytes, NS, KS, p.G4, c.tile, c.tile_end, role, lane, bar_tab, \
+    round_mma<CNT, false>(acc, rp, smem_raw, slot_bytes, tab_bytes, NS, KS, p.G4, c.tile, c.tile_end, role, lane, bar_tab, \
                    bar_seed, bar_done)
-            if constexpr (ScanRegs<H, NOCT, NB>::kAcc > 176) {
+            if (NB == 8 && p.pass > 0) {
+                // a later pass of a multi-pass scan: base families only (NB == 8 is the pass size)
+                round_mma<1, true>(acc, rp, smem_raw, slot_bytes, tab_bytes, NS, KS, p.G4, c.tile, c.tile_end, role, lane,
+                                   bar_tab, bar_seed, bar_done);
+            } else if constexpr (ScanRegs<H, NOCT, NB>::kAcc > 176) {
                 round_mma_pipelined<H, NB>(acc, rp, smem_raw, slot_bytes, tab_bytes, NS, KS, p.G4, c.tile, c.tile_end,
                                            role, lane, bar_tab, bar_seed, bar_done);
             } else if (NOCT == 1 || role.cnt == 1) {
