@@ -625,8 +625,12 @@ __device__ __forceinline__ void solve_and_store(const Tiles<H, NOCT, NB>& acc, c
     const int m = lane >> 2, q = lane & 3;
     const bool last_pass = p.pass + 1 == p.n_pass;
     if (FUSED && info.status != 0) return;  // no periodogram for this series: no lists, no edge records
-    unsigned long long thr_bits = 0;  // fetched before the solves, used after them
-    if constexpr (FUSED) thr_bits = __ldcg(p.group_thr + group);
+    unsigned long long thr_bits = 0;
+    if constexpr (FUSED) {
+        // fetched HERE, before the solves, and used after them: volatile, so that the compiler does not sink
+        // the load to its use and leave the epilogue waiting for a round trip to the L2
+        asm volatile("ld.global.cg.u64 %0, [%1];" : "=l"(thr_bits) : "l"(p.group_thr + group) : "memory");
+    }
 #pragma unroll
     for (int o = 0; o < NOCT; ++o) {
         if (o < cnt) {
