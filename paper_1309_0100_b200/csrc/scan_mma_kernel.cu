@@ -78,8 +78,13 @@ constexpr int kLaunchRegs = 168;  // 65536 / 384 rounded down to the allocation 
 template <int H, int NOCT, int NB>
 struct ScanRegs {
     static constexpr int kAcc = 2 * NOCT * (NB + 2) * H;
+#ifdef FREDEC_EXP_REGS_224_56  // measurement build: 8 registers moved from every MMA thread to the seed warps
+    static constexpr int kMma = kAcc > 176 ? 224 : 216;
+    static constexpr int kSeed = kAcc > 176 ? 56 : 72;
+#else
     static constexpr int kMma = kAcc > 176 ? 232 : 216;
     static constexpr int kSeed = kAcc > 176 ? 40 : 72;
+#endif
     static_assert(kAcc <= 192, "accumulators do not fit the MMA warps' registers");
     static_assert(kNW * kMma + kSeedWarps * kSeed <= (kNW + kSeedWarps) * kLaunchRegs, "register pool exceeded");
 };
