@@ -235,6 +235,36 @@ def run_small_configs(fr, inputs, dev, stream, peak_nominal, with_oracle: bool):
     return out
 
 
+def run_phase1(fr, inputs, dev, with_oracle: bool):
+    """What the scan is for: phase 1 on the RV-like series of config 2 -- residual
+    periodograms with a growing base (d = 1, 3, 5, ...), peaks, statistic and FAP per iteration -- through
+    `fredec_phase1` (device-resident series, one host round trip per iteration), and the oracle's phase 1 on
+    the same arrays: identical pool and base, wall-clock of both."""
+    import torch
+    wl = inputs.config(2)
+    t, x, w, _ = wl.series(0)
+    d_in = [torch.from_numpy(a).to(dev) for a in (t, x, w)]
+    kw = dict(fap0=0.05, fap1=0.1, A1=1.0, max_base=12, k_peaks=32)
+    res = fr.fredec_phase1(*d_in, wl.f0, wl.df, wl.K, **kw)           # warm-up
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    res = fr.fredec_phase1(*d_in, wl.f0, wl.df, wl.K, **kw)
+    torch.cuda.synchronize()
+    ms = 1e3 * (time.perf_counter() - t0)
+    n_it = int(res["base_idx"].size) + 1                               # the last periodogram stops the loop
+    rec = {"workload": f"phase 1 on {wl.name}: N={wl.N} x K={wl.K}, base grows to d={2 * res['base_idx'].size + 1}",
+           "ms": ms, "periodograms": n_it, "launches": fr.fredec_last_launches(),
+           "pool_size": int(res["pool_idx"].size), "base_idx": res["base_idx"].tolist()}
+    if with_oracle:
+        from oracle import phase1 as p1
+        t0 = time.perf_counter()
+        ref = p1.phase1(t, x, w, wl.f0, wl.df, wl.K, fap0=0.05, fap1_thr=0.1, A1=1.0, max_base=12, k_peaks=32, threads=0)
+        rec["oracle_ms"] = 1e3 * (time.perf_counter() - t0)
+        rec["pool_equal_oracle"] = (res["pool_idx"].tolist() == ref["pool_idx"].tolist()
+                                    and res["base_idx"].tolist() == ref["base_idx"].tolist())
+    return rec
+
+
 def main_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -438,6 +468,7 @@ def main_ours(args):
     }
     if world == 1 and not args.no_small_configs:
         line["configs"] = run_small_configs(fr, inputs, dev, stream, peak_nominal, with_oracle=cpu is not None)
+        line["phase1"] = run_phase1(fr, inputs, dev, with_oracle=cpu is not None)
     if multi:
         line["multi_series"] = multi
     if cpu:
