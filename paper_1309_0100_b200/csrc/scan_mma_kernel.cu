@@ -33,9 +33,11 @@
 // observations, one STEP = one tile of TI observations at a time.
 //
 // The CTA is warp-specialised (three warpgroups; registers moved between them with
-// setmaxnreg) around a ring of NS shared-memory slots, slot = (table tile, seeds) of one step:
+// setmaxnreg) around a ring of NS shared-memory slots, slot = (table tile, seeds) of one step
+// (laid out as the NS table tiles followed by the NS seed blocks):
 //
-//   seed warps (4, one per SM sub-partition)  wait until the MMA warps have left the slot
+//   seed warps (4, one per SM sub-partition; the FIRST warpgroup: the scheduler favours them)
+//           wait until the MMA warps have left the slot
 //           (mbarrier "done"); one lane stages the table tile global -> shared by 1-D TMA
 //           (cp.async.bulk, mbarrier "tab"); then a5: seeds e^{i phi} for every (run of the
 //           round, observation of the tile) in A-fragment order -- per lane one exact evaluation
@@ -44,9 +46,11 @@
 //           unit, then the two-term recurrence e_{u+1} = 2 cos(theta) e_u - e_{u-1} along the
 //           units -- and arrive on mbarrier "seed".
 //   MMA warps (8, two per sub-partition)  wait for "tab" and "seed"; per 4 observations:
-//           A fragments (seeds; double-angle seeds by 4 flops), B fragments (table),
+//           A fragments (seeds; double-angle seeds by 2 FP64 instructions), B fragments (table),
 //           2 * NF * NT MMAs per unit; arrive on "done".  After the last tile of a round the
-//           thread that holds all sums of a frequency solves (a9) and stores z (a10).
+//           thread that holds all sums of a frequency solves (a9) and stores z (a10) -- or, in
+//           the FUSED instantiation (no periodogram wanted), tests its values for peaks and
+//           keeps the warp's top-k list (a11, fused_emit).
 //
 // Rounds hold a power of two of units.  A round of fewer units than MMA warps (the tail of a
 // CTA's range, or a short grid) splits the observations between the warps that share a unit
