@@ -235,7 +235,8 @@ int begin_call()
 // fused_k > 0 (peaks only, z_out == nullptr): a11 runs in the scan's epilogue when the scan is a single pass
 // and k <= kFusedMaxK; no periodogram is written then.
 int enqueue_series_mma(Call& c, const double* dt, const double* dx, const double* dw, const double* dbase, int64_t B,
-                       int64_t N, int32_t d, double f0, double df, int64_t K, double* z_out, int32_t fused_k)
+                       int64_t N, int32_t d, double f0, double df, int64_t K, double* z_out, int32_t fused_k,
+                       bool prepped = false)
 {
     cudaStream_t st = g.stream;
     int rc;
@@ -260,14 +261,14 @@ int enqueue_series_mma(Call& c, const double* dt, const double* dx, const double
     pp.info = g.info.as<SeriesInfo>();
     pp.N = N; pp.d = d;
     CK(cudaEventRecord(g.ev[1], st));
-    CK(launch_prep(pp, B, st));
+    if (!prepped) CK(launch_prep(pp, B, st));  // prepped: psi, x~ and the series record are already in place
     TableParams tp;
     tp.t = dt; tp.w = dw; tp.psi = g.psi.as<double>(); tp.xt = g.xt.as<double>();
     tp.info = g.info.as<SeriesInfo>();
     tp.tab = g.tab.as<double>(); tp.srec = g.srec.as<SeedRec>();
     tp.N = N; tp.G4 = G4; tp.d = d; tp.NB = NB; tp.n_pass = n_pass; tp.H = cfg.H; tp.df = df;
     CK(launch_table(tp, B, st));
-    g.launches += 2;
+    g.launches += prepped ? 1 : 2;
     CK(cudaEventRecord(g.ev[2], st));
 
     c.z_count = (size_t)B * K;
@@ -542,6 +543,19 @@ int do_scan(const double* t, const double* x, const double* w, int64_t B, int64_
     return (want_topk && B == 1) ? count : FREDEC_OK;
 }
 
+// One SLICK iteration after the first (fredec_phase1): the base was extended in place by launch_prep_append,
+// so the scan starts at the table kernel.  Single series, device pointers, left pending (deferred).
+int do_scan_prepped(const double* dt, const double* dx, const double* dw, int64_t N, int32_t d, double f0, double df,
+                    int64_t K, double* dz, int32_t k, int64_t* didx)
+{
+    int rc = begin_call();
+    if (rc) return rc;
+    Call c;
+    if ((rc = enqueue_series_mma(c, dt, dx, dw, nullptr, 1, N, d, f0, df, K, dz, 0, true))) return rc;
+    if ((rc = enqueue_topk(c, c.dz, 1, K, k, didx))) return rc;
+    return finish_call(c, nullptr, true);
+}
+
 int do_chi2(const double* t, const double* x, const double* w, int64_t B, int64_t N, const double* base_funcs,
             int32_t d, double* chi2_out)
 {
@@ -736,7 +750,10 @@ int fredec_phase1(const double* t, const double* x, const double* w, int64_t N, 
     const double f_max = f0 + df * (double)(K - 1);
     const double W = f_max * bw[0];  // W = f_max T_eff
 
-    CK(g.p1_base.reserve((size_t)(2 * max_base + 1) * N * 8));
+    CK(g.p1_base.reserve((size_t)N * 8));
+    // the orthonormal base grows in place from iteration to iteration: room for the last one now
+    CK(g.psi.reserve((size_t)(2 * max_base + 1) * N * 8));
+    CK(g.xt.reserve((size_t)N * 8));
     CK(g.p1_freq.reserve((size_t)max_base * 8));
     CK(g.p1_z.reserve((size_t)K * 8));
     CK(g.p1_idx.reserve((size_t)k_peaks * 8));
@@ -753,13 +770,26 @@ int fredec_phase1(const double* t, const double* x, const double* w, int64_t N, 
         const int d = 2 * m + 1;
         const double NH = (double)N - 3.0 * (m + 1) - 1.0;  // N - dim H_{m+1}
         if (NH <= 0.0 || N < (int64_t)d + 3) break;
-        if (m > 0) CK(cudaMemcpyAsync(g.p1_freq.p, base_f.data(), (size_t)m * 8, cudaMemcpyHostToDevice, st));
-        CK(launch_sin_base(dt, N, g.p1_freq.as<double>(), m, g.p1_base.as<double>(), st));
         // one host round trip per iteration: the scan and the peak search are enqueued without a
         // synchronisation, the peak statistics read chi2_base from device memory, and the statuses,
         // indices and statistics come back together
-        int rc1 = do_scan(dt, dx, dw, 1, N, g.p1_base.as<double>(), d, f0, df, K, g.p1_z.as<double>(), k_peaks,
+        int rc1;
+        if (m == 0) {
+            // the constant alone: orthogonalisation from scratch (the prep kernel)
+            CK(launch_sin_base(dt, N, g.p1_freq.as<double>(), 0, g.p1_base.as<double>(), st));
+            rc1 = do_scan(dt, dx, dw, 1, N, g.p1_base.as<double>(), d, f0, df, K, g.p1_z.as<double>(), k_peaks,
                           g.p1_idx.as<int64_t>(), true, true);
+        } else {
+            // the base of the previous iteration plus one sinusoid: the two new functions are appended to
+            // the orthonormal base in place, O(N d) instead of O(N d^2)
+            CK(cudaMemcpyAsync(g.p1_freq.as<double>() + (m - 1), &base_f[m - 1], 8, cudaMemcpyHostToDevice, st));
+            PrepAppendParams ap;
+            ap.t = dt; ap.w = dw; ap.freq = g.p1_freq.as<double>() + (m - 1);
+            ap.psi = g.psi.as<double>(); ap.xt = g.xt.as<double>(); ap.info = g.info.as<SeriesInfo>();
+            ap.N = N; ap.d0 = d - 2;
+            CK(launch_prep_append(ap, st));
+            rc1 = do_scan_prepped(dt, dx, dw, N, d, f0, df, K, g.p1_z.as<double>(), k_peaks, g.p1_idx.as<int64_t>());
+        }
         launches += 1 + g.launches;
         if (rc1 < 0) return rc1;
         CK(launch_peak_stats(g.p1_z.as<double>(), g.p1_idx.as<int64_t>(), k_peaks, g.info.as<SeriesInfo>(), NH, W, A1,

@@ -432,6 +432,172 @@ __global__ void __launch_bounds__(kPrepThreads) prep_kernel(PrepParams p, int sp
 #endif
 }
 
+// ---- a2, incremental form (the base model of the next SLICK iteration is the current one plus
+// one sinusoid) -------------------------------------------------------------------------------
+// psi_0 .. psi_{d0-1} are orthonormal and x~ is the residual of x after them (the previous prep / append).
+// The two new base functions cos / sin(2 pi f t) are orthogonalised against them by two rounds of projection
+// ("twice is enough"), then against each other and normalised (a 2 x 2 Cholesky step), appended
+// as rows d0 and d0 + 1 of psi, and x~ and chi2_base are updated: O(N d) instead of the O(N d^2) of a prep from
+// scratch.  One CTA (the driver's series is a single one), fixed-order sums.
+constexpr int kAppendThreads = 512;
+constexpr int kAppendWarps = kAppendThreads / 32;
+
+// NV fixed-order block sums at once (one barrier pair): `red` = NV * kAppendWarps doubles.
+template <int NV>
+__device__ void append_block_sum(double (&v)[NV], double* red)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+        for (int k = 0; k < NV; ++k) v[k] += __shfl_xor_sync(0xffffffffu, v[k], o);
+    __syncthreads();
+    if (lane == 0)
+#pragma unroll
+        for (int k = 0; k < NV; ++k) red[k * kAppendWarps + wid] = v[k];
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+        double r = 0.0;
+        for (int q = 0; q < kAppendWarps; ++q) r += red[k * kAppendWarps + q];
+        v[k] = r;
+    }
+}
+
+__global__ void __launch_bounds__(kAppendThreads) prep_append_kernel(PrepAppendParams p)
+{
+    extern __shared__ __align__(16) double coef[];  // [2][d0]
+    __shared__ double red[5 * kAppendWarps];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int64_t N = p.N;
+    const int d0 = p.d0;
+    double* pa = p.psi + (int64_t)d0 * N;  // the two new rows, worked on in place
+    double* pb = pa + N;
+    SeriesInfo* info = p.info;
+    if (info->status != 0) return;  // uniform: the series already failed
+    const double f = *p.freq;
+    // the new functions (phase reduced exactly, as the base builder of the from-scratch path does)
+    double n0a = 0.0, n0b = 0.0;
+    for (int64_t i = threadIdx.x; i < N; i += kAppendThreads) {
+        double sv, cv;
+        sincospi(2.0 * frac_prod(f, p.t[i]), &sv, &cv);
+        pa[i] = cv;
+        pb[i] = sv;
+        const double wi = p.w[i];
+        n0a = fma(wi * cv, cv, n0a);
+        n0b = fma(wi * sv, sv, n0b);
+    }
+    {
+        double v[2] = {n0a, n0b};
+        append_block_sum(v, red);
+        n0a = v[0];
+        n0b = v[1];
+    }
+    for (int round = 0; round < 2; ++round) {
+        __syncthreads();
+        for (int j = wid; j < d0; j += kAppendWarps) {
+            const double* pj = p.psi + (int64_t)j * N;
+            double c = 0.0, e = 0.0, c1 = 0.0, e1 = 0.0;
+            int64_t i = lane;
+            for (; i + 96 < N; i += 128) {  // four independent loads of each array in flight
+                const double w0 = p.w[i] * pj[i], w1 = p.w[i + 32] * pj[i + 32];
+                const double w2 = p.w[i + 64] * pj[i + 64], w3 = p.w[i + 96] * pj[i + 96];
+                c = fma(w0, pa[i], c);
+                e = fma(w0, pb[i], e);
+                c1 = fma(w1, pa[i + 32], c1);
+                e1 = fma(w1, pb[i + 32], e1);
+                c = fma(w2, pa[i + 64], c);
+                e = fma(w2, pb[i + 64], e);
+                c1 = fma(w3, pa[i + 96], c1);
+                e1 = fma(w3, pb[i + 96], e1);
+            }
+            for (; i < N; i += 32) {
+                const double wp = p.w[i] * pj[i];
+                c = fma(wp, pa[i], c);
+                e = fma(wp, pb[i], e);
+            }
+            c += c1;
+            e += e1;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                c += __shfl_xor_sync(0xffffffffu, c, o);
+                e += __shfl_xor_sync(0xffffffffu, e, o);
+            }
+            if (lane == 0) {
+                coef[j] = c;
+                coef[d0 + j] = e;
+            }
+        }
+        __syncthreads();
+        for (int64_t i = threadIdx.x; i < N; i += kAppendThreads) {
+            double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0;
+            int j = 0;
+            for (; j + 1 < d0; j += 2) {
+                const double v0 = p.psi[(int64_t)j * N + i], v1 = p.psi[(int64_t)(j + 1) * N + i];
+                a0 = fma(coef[j], v0, a0);
+                a1 = fma(coef[j + 1], v1, a1);
+                b0 = fma(coef[d0 + j], v0, b0);
+                b1 = fma(coef[d0 + j + 1], v1, b1);
+            }
+            if (j < d0) {
+                const double v0 = p.psi[(int64_t)j * N + i];
+                a0 = fma(coef[j], v0, a0);
+                b0 = fma(coef[d0 + j], v0, b0);
+            }
+            pa[i] -= a0 + a1;
+            pb[i] -= b0 + b1;
+        }
+    }
+    __syncthreads();
+    // the 2 x 2 step: Gram of (phi_a, phi_b) with x~ carried as the right-hand side
+    double naa = 0.0, nab = 0.0, nbb = 0.0, xa = 0.0, xb = 0.0;
+    for (int64_t i = threadIdx.x; i < N; i += kAppendThreads) {
+        const double wi = p.w[i], a = pa[i], b = pb[i], xw = wi * p.xt[i];
+        naa = fma(wi * a, a, naa);
+        nab = fma(wi * a, b, nab);
+        nbb = fma(wi * b, b, nbb);
+        xa = fma(xw, a, xa);
+        xb = fma(xw, b, xb);
+    }
+    {
+        double v[5] = {naa, nab, nbb, xa, xb};
+        append_block_sum(v, red);
+        naa = v[0]; nab = v[1]; nbb = v[2]; xa = v[3]; xb = v[4];
+    }
+    int status = 0;
+    double ra = 0.0, rb = 0.0, q = 0.0;
+    if (naa > kTauBase * n0a) {  // else: the cosine is in the span of the base (S6b)
+        ra = rsqrt(naa);
+        q = nab * ra;
+    } else {
+        status = -3;
+    }
+    const double nbb2 = nbb - q * q;
+    if (status == 0 && nbb2 > kTauBase * n0b)
+        rb = rsqrt(nbb2);
+    else
+        status = -3;
+    const double aa = xa * ra, ab = (xb - q * aa) * rb;
+    double chi2 = 0.0;
+    for (int64_t i = threadIdx.x; i < N; i += kAppendThreads) {
+        const double va = pa[i] * ra, vb = (pb[i] - q * va) * rb;
+        pa[i] = va;
+        pb[i] = vb;
+        const double xv = p.xt[i] - fma(aa, va, ab * vb);
+        p.xt[i] = xv;
+        chi2 = fma(p.w[i] * xv, xv, chi2);
+    }
+    {
+        double v[1] = {chi2};
+        append_block_sum(v, red);
+        chi2 = v[0];
+    }
+    if (threadIdx.x == 0) {
+        info->chi2_base = status == 0 ? chi2 : 0.0;
+        info->status = status;
+    }
+}
+
 // ---- a3: per-observation table and seed records --------------------------
 // One thread per (observation, pair of column tiles tp, position hh in a tile): two grid offsets h and h + 4,
 // four sincospi of exactly reduced phases, and the entries of every family for them.  The series are
@@ -498,6 +664,13 @@ cudaError_t launch_table(const TableParams& p, int64_t B, cudaStream_t stream)
     dim3 grid((unsigned)((p.G4 * 4 + kTableObs - 1) / kTableObs), (unsigned)p.n_pass, (unsigned)B);
     dim3 block(kTableObs, (unsigned)(mma_nt(p.H) / 2 * 4));  // at most 32 x 24 threads (H = 48)
     table_kernel<<<grid, block, 0, stream>>>(p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_prep_append(const PrepAppendParams& p, cudaStream_t stream)
+{
+    const size_t smem = (size_t)2 * (p.d0 > 0 ? p.d0 : 1) * sizeof(double);
+    prep_append_kernel<<<1, kAppendThreads, smem, stream>>>(p);
     return cudaGetLastError();
 }
 

@@ -35,4 +35,18 @@ cudaError_t launch_table(const TableParams& p, int64_t B, cudaStream_t stream);
 
 cudaError_t launch_prep(const PrepParams& p, int64_t B, cudaStream_t stream);
 
+// Incremental a2 for one series: appends cos / sin(2 pi f t) to the orthonormal base psi [d0][N] (rows d0 and
+// d0 + 1 must be allocated) and updates x~ and chi2_base; see prep_kernel.cu.
+struct PrepAppendParams {
+    const double* t;     // [N]
+    const double* w;     // [N]
+    const double* freq;  // device pointer to the new frequency
+    double* psi;         // [d0 + 2][N]
+    double* xt;          // [N]
+    SeriesInfo* info;
+    int64_t N;
+    int d0;
+};
+cudaError_t launch_prep_append(const PrepAppendParams& p, cudaStream_t stream);
+
 }  // namespace fredec
