@@ -555,23 +555,34 @@ __device__ __forceinline__ void fused_emit(double (&zu)[H / 4], double (&zl)[H /
     constexpr unsigned kFull = 0xffffffffu;
     const int m = lane >> 2, q = lane & 3, quad = lane & ~3;
     const int64_t k0 = (unit * 8 + m) * R;
-    // points past the end of the grid and NaN count as -infinity (S7)
-    double vmax = -INFINITY;
+    // points past the end of the grid count as -infinity (S7): only the last unit of a series has any
+    if ((unit + 1) * 8 * R > p.K) {
+#pragma unroll
+        for (int t = 0; t < NT; ++t) {
+            if (k0 + H + 4 * t + q >= p.K) zu[t] = -INFINITY;
+            if (k0 + H - 1 - 4 * t - q >= p.K) zl[t] = -INFINITY;
+        }
+    }
+    // edge record: the half of the peak test that the unit can decide (NaN counts as -infinity)
+    const double z_first = sanitize(zl[NT - 1]), z_last = sanitize(zu[NT - 1]);
+    const double right_of_first = __shfl_sync(kFull, z_first, 2);  // run 0, position 1
+    const double left_of_last = __shfl_sync(kFull, z_last, 30);    // run 7, position R - 2
+    double2* er = reinterpret_cast<double2*>(p.edges + (b * p.U + unit) * 4);
+    if (lane == 3) __stcg(er, make_double2(z_first, z_first >= right_of_first ? 1.0 : 0.0));
+    if (lane == 31) __stcg(er + 1, make_double2(z_last, z_last > left_of_last ? 1.0 : 0.0));
+    // nothing at or above the group's threshold (the largest k-th entry of its full lists): no candidate.
+    // One comparison per value and one vote (a NaN compares false) -- the common case must stay cheap: its
+    // FP64 instructions compete with the MMAs of the sub-partition's other warp.
+    const double group_thr = thr_bits ? __longlong_as_double((long long)thr_bits) : -INFINITY;
+    bool reach = false;
+#pragma unroll
+    for (int t = 0; t < NT; ++t) reach |= (zu[t] >= group_thr) | (zl[t] >= group_thr);
+    if (!__any_sync(kFull, reach)) return;
 #pragma unroll
     for (int t = 0; t < NT; ++t) {
-        zu[t] = k0 + H + 4 * t + q < p.K ? sanitize(zu[t]) : -INFINITY;
-        zl[t] = k0 + H - 1 - 4 * t - q < p.K ? sanitize(zl[t]) : -INFINITY;
-        vmax = fmax(vmax, fmax(zu[t], zl[t]));
+        zu[t] = sanitize(zu[t]);
+        zl[t] = sanitize(zl[t]);
     }
-    // edge record: the half of the peak test that the unit can decide
-    const double right_of_first = __shfl_sync(kFull, zl[NT - 1], 2);  // run 0, position 1
-    const double left_of_last = __shfl_sync(kFull, zu[NT - 1], 30);   // run 7, position R - 2
-    double2* er = reinterpret_cast<double2*>(p.edges + (b * p.U + unit) * 4);
-    if (lane == 3) __stcg(er, make_double2(zl[NT - 1], zl[NT - 1] >= right_of_first ? 1.0 : 0.0));
-    if (lane == 31) __stcg(er + 1, make_double2(zu[NT - 1], zu[NT - 1] > left_of_last ? 1.0 : 0.0));
-    // nothing at or above the group's threshold (the largest k-th entry of its full lists): no candidate
-    const double group_thr = thr_bits ? __longlong_as_double((long long)thr_bits) : -INFINITY;
-    if (!__any_sync(kFull, vmax >= group_thr)) return;
     // the warp's list
     const int k = p.fused_k;
     double* lz = p.list_z + ((size_t)group * kNW + w) * k;
