@@ -566,6 +566,7 @@ def main():
     ap.add_argument("--profile-k", type=int, default=0, help="with --profile-config: override K")
     ap.add_argument("--profile-nbase", type=int, default=0, help="with --profile-config 3: sinusoids in the base")
     ap.add_argument("--profile-no-z", action="store_true", help="with --profile-config: peaks only (z_out = NULL)")
+    ap.add_argument("--profile-phase1", action="store_true", help="run only the phase-1 block (for ncu launch lists) and exit")
     args = ap.parse_args()
     if args.steps < 1:
         ap.error("--steps must be >= 1")
@@ -573,6 +574,16 @@ def main():
         return main_fp64_probe(args)
     if args.profile_config:
         return main_profile(args)
+    if args.profile_phase1:
+        import torch
+        from paper_1309_0100_b200 import build as lib_build
+        lib_build.build()
+        import paper_1309_0100_b200 as fr
+        from paper_1309_0100_b200 import inputs
+        torch.cuda.set_device(0)
+        fr.fredec_set_stream(torch.cuda.current_stream())
+        print(json.dumps(run_phase1(fr, inputs, torch.device("cuda", 0), with_oracle=False)))
+        return 0
     return main_reference(args) if args.impl == "reference" else main_ours(args)
 
 
