@@ -195,8 +195,9 @@ def run_small_configs(fr, inputs, dev, stream, peak_nominal, with_oracle: bool):
         b.record(stream)
         torch.cuda.synchronize()
         step_ms = a.elapsed_time(b) / steps
-        # the asynchronous form: no host round trip between the steps
+        # the asynchronous form without the per-stage timing events: no host round trip between the steps
         fr.fredec_set_async(True)
+        fr.fredec_set_timing(False)
         try:
             step()
             torch.cuda.synchronize()
@@ -208,6 +209,7 @@ def run_small_configs(fr, inputs, dev, stream, peak_nominal, with_oracle: bool):
             fr.fredec_last_status()
         finally:
             fr.fredec_set_async(False)
+            fr.fredec_set_timing(True)
         async_ms = a.elapsed_time(b) / steps
         F = flops_per_pair(wl.d)
         rec = {"workload": f"{wl.name}: N={wl.N} x K={wl.K}, d={wl.d}, top-{wl.topk}", "pairs": wl.pairs,

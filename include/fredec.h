@@ -284,6 +284,13 @@ int fredec_last_status(int32_t* count_out);
  * out[2] = top-k kernel(s), out[3] = whole call including staging copies. Unused = 0. */
 int fredec_last_timing(double out[4]);
 
+/*
+ * fredec_set_timing -- enable == 0: the scan / top-k calls stop recording the per-stage CUDA events behind
+ * fredec_last_timing (seven event records per call, about 25 microseconds of host time: what a call on a
+ * small series costs otherwise); fredec_last_timing then reports zeros.  enable != 0 (default): recorded.
+ */
+int fredec_set_timing(int32_t enable);
+
 /* Number of kernels the LAST compute call launched. */
 int fredec_last_launches(void);
 

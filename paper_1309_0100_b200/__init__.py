@@ -7,7 +7,7 @@ from ._binding import (  # noqa: F401
     FREDEC_D_MAX, FREDEC_ECUDA, FREDEC_EDATA, FREDEC_EINVAL, FREDEC_ESINGULAR, FREDEC_OK,
     FREDEC_TOPK_MAX, FredecError, LIB_PATH,
     fredec_chi2_base, fredec_chi2_base_batched, fredec_bench_fp64, fredec_bench_fp64_name, fredec_last_launches,
-    fredec_last_timing, fredec_scan, fredec_scan_batched, fredec_scan_topk, fredec_scan_topk_batched, fredec_set_stream, fredec_set_async, fredec_last_status, fredec_shutdown,
+    fredec_last_timing, fredec_scan, fredec_scan_batched, fredec_scan_topk, fredec_scan_topk_batched, fredec_set_stream, fredec_set_async, fredec_set_timing, fredec_last_status, fredec_shutdown,
     fredec_topk, fredec_topk_batched, fredec_version, lib,
     fredec_bandwidth, fredec_fap1, fredec_phase1, fredec_refine, fredec_refine_batched, fredec_subset_fits, fredec_trig_averages, fredec_zstat,
 )

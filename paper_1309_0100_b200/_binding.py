@@ -42,6 +42,7 @@ SIGNATURES = {
     "fredec_refine_batched": (C.c_int, [_P, _P, _P, _I64, _P, _I32, _P, _I64, _I32, _F64, _P, _P, _P, _P]),
     "fredec_set_stream": (C.c_int, [_P]),
     "fredec_set_async": (C.c_int, [_I32]),
+    "fredec_set_timing": (C.c_int, [_I32]),
     "fredec_last_status": (C.c_int, [C.POINTER(C.c_int32)]),
     "fredec_last_timing": (C.c_int, [C.POINTER(C.c_double)]),
     "fredec_last_launches": (C.c_int, []),
@@ -124,6 +125,11 @@ def fredec_set_stream(stream=None) -> None:
 def fredec_set_async(enable: bool) -> None:
     """Asynchronous form for scan / top-k calls on device pointers; see include/fredec.h."""
     _check(lib().fredec_set_async(1 if enable else 0), "fredec_set_async")
+
+
+def fredec_set_timing(enable: bool) -> None:
+    """Per-stage CUDA-event timing of the scan / top-k calls (fredec_last_timing) on or off."""
+    _check(lib().fredec_set_timing(1 if enable else 0), "fredec_set_timing")
 
 
 def fredec_last_status() -> int:

@@ -95,8 +95,18 @@ struct State {
     bool pend_series = false, pend_topk = false;
     int64_t pend_B = 0;
     int last_status = 0, last_count = 0;
+    // the per-stage timing events of the scan / top-k calls; off inside fredec_phase1, whose iterations are
+    // short enough for seven event records each to show
+    bool timing_on = true;
 };
 State g;
+
+cudaError_t record_event(int i) { return g.timing_on ? cudaEventRecord(g.ev[i], g.stream) : cudaSuccess; }
+struct TimingOff {
+    bool before;
+    TimingOff() : before(g.timing_on) { g.timing_on = false; }
+    ~TimingOff() { g.timing_on = before; }
+};
 
 // Error path of every entry point: copies or kernels that touch the caller's buffers may still be
 // queued on the stream; wait for them so that "the library keeps no pointer after return" also holds
@@ -227,7 +237,7 @@ int begin_call()
     if (g.pending) (void)resolve_pending();  // its events and pinned status buffers are about to be reused
     g.launches = 0;
     for (double& v : g.timing) v = 0.0;
-    CK(cudaEventRecord(g.ev[0], g.stream));
+    CK(record_event(0));
     return FREDEC_OK;
 }
 
@@ -260,7 +270,7 @@ int enqueue_series_mma(Call& c, const double* dt, const double* dx, const double
     pp.psi = g.psi.as<double>(); pp.xt = g.xt.as<double>();
     pp.info = g.info.as<SeriesInfo>();
     pp.N = N; pp.d = d;
-    CK(cudaEventRecord(g.ev[1], st));
+    CK(record_event(1));
     if (!prepped) CK(launch_prep(pp, B, st));  // prepped: psi, x~ and the series record are already in place
     TableParams tp;
     tp.t = dt; tp.w = dw; tp.psi = g.psi.as<double>(); tp.xt = g.xt.as<double>();
@@ -269,7 +279,7 @@ int enqueue_series_mma(Call& c, const double* dt, const double* dx, const double
     tp.N = N; tp.G4 = G4; tp.d = d; tp.NB = NB; tp.n_pass = n_pass; tp.H = cfg.H; tp.df = df;
     CK(launch_table(tp, B, st));
     g.launches += prepped ? 1 : 2;
-    CK(cudaEventRecord(g.ev[2], st));
+    CK(record_event(2));
 
     c.z_count = (size_t)B * K;
     const bool fused = z_out == nullptr && fused_k > 0 && fused_k <= kFusedMaxK && n_pass == 1;
@@ -364,7 +374,7 @@ int enqueue_series_mma(Call& c, const double* dt, const double* dx, const double
         CK(launch_mma_scan(NB, sp, st));
         g.launches += (sp.shared && sp.Rt > 0) ? 2 : 1;  // + the tail-solve kernel
     }
-    CK(cudaEventRecord(g.ev[3], st));
+    CK(record_event(3));
     c.B = B;
     c.has_series = true;
     return FREDEC_OK;
@@ -398,11 +408,11 @@ int enqueue_series(Call& c, const double* t, const double* x, const double* w, i
     pp.psi = g.psi.as<double>(); pp.xt = g.xt.as<double>();
     pp.info = g.info.as<SeriesInfo>();
     pp.N = N; pp.d = d;
-    CK(cudaEventRecord(g.ev[1], st));
+    CK(record_event(1));
     CK(launch_prep(pp, B, st));
     g.launches += 1;
-    CK(cudaEventRecord(g.ev[2], st));
-    CK(cudaEventRecord(g.ev[3], st));
+    CK(record_event(2));
+    CK(record_event(3));
     c.B = B;
     c.has_series = true;
     return FREDEC_OK;
@@ -428,11 +438,11 @@ int enqueue_topk(Call& c, const double* dz, int64_t B, int64_t K, int32_t k, int
         tp.part_z = g.part_z.as<double>();
         tp.part_i = g.part_i.as<int64_t>();
     }
-    CK(cudaEventRecord(g.ev[4], st));
+    CK(record_event(4));
     int nl = 0;
     CK(launch_topk(tp, B, st, &nl));
     g.launches += nl;
-    CK(cudaEventRecord(g.ev[5], st));
+    CK(record_event(5));
     c.B = B;
     c.has_topk = true;
     return FREDEC_OK;
@@ -449,10 +459,10 @@ int enqueue_fused_merge(Call& c, int64_t B, int32_t k, int64_t* idx_out)
     CK(g.h_count.reserve((size_t)B * sizeof(int)));
     c.fm.idx_out = c.didx;
     c.fm.count_out = g.count.as<int>();
-    CK(cudaEventRecord(g.ev[4], st));
+    CK(record_event(4));
     CK(launch_fused_merge(c.fm, B, st));
     g.launches += 1;
-    CK(cudaEventRecord(g.ev[5], st));
+    CK(record_event(5));
     c.has_topk = true;
     return FREDEC_OK;
 }
@@ -466,12 +476,14 @@ int resolve_pending()
     g.last_status = FREDEC_ECUDA;
     g.last_count = 0;
     CK(cudaStreamSynchronize(g.stream));
-    if (g.pend_series) {
-        g.timing[0] = ev_ms(1, 2);
-        g.timing[1] = ev_ms(2, 3);
+    if (g.timing_on) {
+        if (g.pend_series) {
+            g.timing[0] = ev_ms(1, 2);
+            g.timing[1] = ev_ms(2, 3);
+        }
+        if (g.pend_topk) g.timing[2] = ev_ms(4, 5);
+        g.timing[3] = ev_ms(0, 6);
     }
-    if (g.pend_topk) g.timing[2] = ev_ms(4, 5);
-    g.timing[3] = ev_ms(0, 6);
     g.last_status = FREDEC_OK;
     if (g.pend_series) {
         const SeriesInfo* hi = static_cast<const SeriesInfo*>(g.h_info.p);
@@ -496,7 +508,7 @@ int finish_call(Call& c, int* first_count, bool defer = false)
         CK(cudaMemcpyAsync(g.h_info.p, g.info.p, (size_t)c.B * sizeof(SeriesInfo), cudaMemcpyDeviceToHost, st));
     if (c.has_topk)
         CK(cudaMemcpyAsync(g.h_count.p, g.count.p, (size_t)c.B * sizeof(int), cudaMemcpyDeviceToHost, st));
-    CK(cudaEventRecord(g.ev[6], st));
+    CK(record_event(6));
     g.pending = true;
     g.pend_series = c.has_series;
     g.pend_topk = c.has_topk;
@@ -739,6 +751,7 @@ int fredec_phase1(const double* t, const double* x, const double* w, int64_t N, 
     if (on_device(pool_idx) || on_device(pool_z) || on_device(pool_fap) || on_device(base_idx)) return FREDEC_EINVAL;
     if ((rc = ensure_ready())) return rc;
     cudaStream_t st = g.stream;
+    TimingOff no_stage_timing;
 
     // the series stays on the device for all iterations
     const double *dt, *dx, *dw;
@@ -1003,6 +1016,13 @@ int fredec_last_timing(double out[4])
     if (!out) return FREDEC_EINVAL;
     if (g.pending) (void)resolve_pending();
     for (int i = 0; i < 4; ++i) out[i] = g.timing[i];
+    return FREDEC_OK;
+}
+
+int fredec_set_timing(int32_t enable)
+{
+    if (g.pending) (void)resolve_pending();
+    g.timing_on = enable != 0;
     return FREDEC_OK;
 }
 

@@ -328,6 +328,27 @@ def test_asynchronous_form(fr, oracle_mod):
     assert fr.fredec_scan_topk(dt, dx, dw, db, wl.f0, wl.df, wl.K, 10)[2] == cnt_sync
 
 
+def test_stage_timing_switch(fr):
+    """fredec_set_timing (include/fredec.h): without the per-stage events the results are the same bits and
+    fredec_last_timing reports zeros; switched back on, the stages are timed again."""
+    import torch
+    wl = inputs.config(1)
+    t, x, w, base = wl.series(0)
+    dt, dx, dw, db = _dev(t, x, w, base)
+    z_on, idx_on, cnt_on = fr.fredec_scan_topk(dt, dx, dw, db, wl.f0, wl.df, wl.K, 10)
+    assert fr.fredec_last_timing()["scan_ms"] > 0.0
+    fr.fredec_set_timing(False)
+    try:
+        z_off, idx_off, cnt_off = fr.fredec_scan_topk(dt, dx, dw, db, wl.f0, wl.df, wl.K, 10)
+        tm = fr.fredec_last_timing()
+        assert tm["scan_ms"] == 0.0 and tm["total_ms"] == 0.0
+        assert cnt_off == cnt_on and torch.equal(z_off, z_on) and torch.equal(idx_off, idx_on)
+    finally:
+        fr.fredec_set_timing(True)
+    fr.fredec_scan_topk(dt, dx, dw, db, wl.f0, wl.df, wl.K, 10)
+    assert fr.fredec_last_timing()["scan_ms"] > 0.0
+
+
 def test_large_phase_accuracy(fr, oracle_mod):
     """t ~ 2.4e6 (Julian-date like), f up to 20: phases of ~5e7 turns."""
     t, x, w, _ = inputs.random_series(77, 400, 0, t_span=300.0)
