@@ -791,6 +791,9 @@ __global__ void __launch_bounds__(kThreads, 1) scan_mma_kernel(MmaScanParams p)
 
     Cursor c;
     c.init(p, ntiles, CAP);
+    // the tail-solve kernel (launched with programmatic stream serialisation) may be scheduled as soon as SMs
+    // become free; it waits for this grid's completion before it reads anything
+    asm volatile("griddepcontrol.launch_dependents;");
 
     if (seed_warp) {
         // ================= seed warps: table staging (a4) + seeds (a5) =====================
@@ -971,6 +974,9 @@ __global__ void __launch_bounds__(kNW * 32) tail_solve_kernel(MmaScanParams p)
     const int64_t r = blockIdx.x, S = (int64_t)p.Rt * ntiles;
     Tiles<H, NOCT, NB> acc;
     acc.clear();
+    // launched with programmatic stream serialisation: everything above overlaps the scan kernel's end; the
+    // partial sums are read only after the scan kernel has completed and flushed
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     // only the CTAs whose piece [cta S / grid, (cta + 1) S / grid) can meet the round's steps [r, r + 1) ntiles
     const int c_lo = (int)max((int64_t)0, r * ntiles * p.grid / S - 1);
     const int c_hi = (int)min((int64_t)p.grid - 1, ((r + 1) * ntiles * p.grid + S - 1) / S);
@@ -1012,8 +1018,17 @@ cudaError_t launch_one(const MmaScanParams& p, cudaStream_t stream)
     scan_mma_kernel<H, NOCT, NB, FUSED><<<p.grid, kThreads, smem, stream>>>(p);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess || !p.shared || p.Rt == 0) return e;
-    tail_solve_kernel<H, NOCT, NB, FUSED><<<p.Rt, kNW * 32, 0, stream>>>(p);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)p.Rt, 1, 1);
+    cfg.blockDim = dim3(kNW * 32, 1, 1);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, tail_solve_kernel<H, NOCT, NB, FUSED>, p);
 }
 
 }  // namespace
