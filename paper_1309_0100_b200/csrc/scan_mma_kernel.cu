@@ -527,6 +527,9 @@ __device__ __forceinline__ void round_mma(Tiles<H, NOCT, NB>& acc, RingPos& rp, 
 __device__ __forceinline__ double solve_z(double YC, double YS, double CC, double CS, double Saa, double Sab,
                                           double Sbb, double W)
 {
+#ifdef FREDEC_EXP_NO_SOLVE  // measurement build (wrong results): what the Schur solves cost
+    return YC + YS + CC + CS + Saa + Sab + Sbb + W;
+#endif
     const double SS = W - CC;  // <sin^2> = <1> - <cos^2>
     const double Scc = CC - Saa, Scs = CS - Sab, Sss = SS - Sbb;
     // two reciprocals instead of three divisions: the epilogue's FP64 instructions run while no MMA does
