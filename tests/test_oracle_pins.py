@@ -350,3 +350,39 @@ def test_topk_config1_sanity(oracle_mod):
     idx, cnt = oracle_mod.topk(z, 10)
     assert cnt == 10 and abs(idx[0] - 568) <= 1 and abs(idx[1] - 100) <= 1
     assert np.all(np.diff(z[idx]) <= 0)
+
+
+@pytest.mark.parametrize("seed,K", [(1, 3000), (2, 257), (3, 20_000)])
+def test_topk_against_scipy_find_peaks(oracle_mod, seed, K):
+    """oracle_topk against a library peak finder it shares nothing with: on an array without ties the peaks of
+    reading S7 (z[i] > z[i-1] and z[i] >= z[i+1], outside = -infinity) are scipy.signal.find_peaks' strict
+    interior maxima plus an end point that tops its one neighbour; the order is z descending; a k below the
+    number of peaks keeps the k highest."""
+    from scipy.signal import find_peaks
+    rng = np.random.Generator(np.random.PCG64(1000 + seed))
+    z = rng.standard_normal(K).cumsum() * 0.05 + rng.standard_normal(K)
+    ref = set(find_peaks(z)[0].tolist())
+    if z[0] >= z[1]:
+        ref.add(0)
+    if z[-1] > z[-2]:
+        ref.add(K - 1)
+    idx, cnt = oracle_mod.topk(z, K)
+    got = idx[:cnt]
+    assert cnt == len(ref) and set(got.tolist()) == ref and np.all(idx[cnt:] == -1)
+    assert np.all(np.diff(z[got]) <= 0.0)
+    k = max(1, cnt // 7)
+    idx_k, cnt_k = oracle_mod.topk(z, k)
+    assert cnt_k == k and idx_k.tolist() == got[:k].tolist()
+    # ties: S7 takes the first point of a flat stretch reached by an ascent -- of a plateau that tops both sides
+    # (find_peaks reports its middle) and, by the letter of the rule, also of a shelf on an ascending slope
+    zp = np.round(z, 1)
+    mid, props = find_peaks(zp, plateau_size=1)
+    idx_p, cnt_p = oracle_mod.topk(zp, K)
+    got_p = set(idx_p[:cnt_p].tolist())
+    assert set(props["left_edges"].tolist()) <= got_p
+    for i in got_p - set(props["left_edges"].tolist()) - {0, K - 1}:
+        j = i
+        while j + 1 < K and zp[j + 1] == zp[i]:
+            j += 1
+        assert zp[i - 1] < zp[i] and j > i and (j + 1 == K or zp[j + 1] > zp[i]), i   # a shelf, or a final plateau
+    assert oracle_mod.topk(np.array([1.0, 2.0, 2.0, 3.0, 0.0]), 5)[0].tolist() == [3, 1, -1, -1, -1]
