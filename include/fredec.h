@@ -49,9 +49,12 @@ extern "C" {
 #define FREDEC_EDATA (-2)     /* non-finite t/x/w/base value, w_i < 0, sum w = 0 */
 #define FREDEC_ESINGULAR (-3) /* base functions linearly dependent (S6b) */
 #define FREDEC_ECUDA (-4)     /* CUDA runtime error; see fredec_last_cuda_error() */
+#define FREDEC_ELIMIT (-5)    /* a size exceeds the fixed capacity of an entry point that owns no growable
+                                 memory (fredec_topk_noalloc: k > FREDEC_TOPK_NOALLOC_K_MAX) */
 
 #define FREDEC_D_MAX 64       /* the paper's pools reach n = 25 sinusoids => d = 51 */
 #define FREDEC_TOPK_MAX 1024
+#define FREDEC_TOPK_NOALLOC_K_MAX 128 /* longest peak list of fredec_topk_noalloc (its scratch array is fixed) */
 
 /*
  * fredec_scan -- periodogram scan (section 4.2 "single-frequency residual
@@ -110,6 +113,48 @@ int fredec_chi2_base_batched(const double* t, const double* x, const double* w, 
  */
 int fredec_topk(const double* z, int64_t K, int32_t k, int64_t* idx_out);
 int fredec_topk_batched(const double* z, int64_t B, int64_t K, int32_t k, int64_t* idx_out);
+
+/*
+ * fredec_topk_noalloc -- fredec_topk for callers that must not allocate device memory (same operation:
+ * PAPER.md:201-206, reading S7; same indices bit for bit).
+ *
+ * Why it exists.  fredec_topk keeps a library-owned workspace that it grows with cudaMalloc when a larger
+ * problem arrives, and pinned host memory for the count it returns.  That is wrong for a program that has
+ * given the whole GPU to its own memory pool (the library's cudaMalloc then reports out-of-memory while the
+ * pool sits half empty), for a service that cannot take the device-wide stall a cudaMalloc / cudaFree
+ * causes on all its streams, and for code running where the CUDA allocator is off limits.  This entry point
+ * never calls cudaMalloc, cudaFree, cudaMallocHost or any allocating library routine.  Its only scratch
+ * memory is an array compiled into the library: fredec_topk_noalloc_scratch_bytes() bytes (about 1.2 MB)
+ * that every GPU which loads libfredec_b200.so holds until the process exits.
+ *
+ *   z [K]          DEVICE pointer (device or managed memory of the current device), input, not modified
+ *   K >= 1;  1 <= k <= min(K, FREDEC_TOPK_NOALLOC_K_MAX)
+ *   idx_out [k]    DEVICE pointer: indices of the k highest peaks, z descending then index ascending,
+ *                  unused slots -1
+ *   count_out [1]  DEVICE pointer (int32): number of peaks written, 0..k
+ *   cuda_stream    a cudaStream_t passed as void* (NULL: the default stream); fredec_set_stream does not
+ *                  apply here.  The work (one 256-byte memset and one kernel) is enqueued on it and the
+ *                  call returns without waiting: the outputs are ready once the caller has synchronised
+ *                  with that stream.
+ *
+ * Returns FREDEC_OK; FREDEC_EINVAL for a NULL pointer, K < 1, k < 1, k > K, or a pointer that is not
+ * device-accessible (host buffers would need staging memory, which this call may not allocate);
+ * FREDEC_ELIMIT for k > FREDEC_TOPK_NOALLOC_K_MAX -- use fredec_topk for longer lists;
+ * FREDEC_ECUDA for a CUDA error, whose cudaError_t fredec_topk_noalloc_cuda_error() returns.
+ * There is no limit on K.
+ *
+ * Rules that follow from the shared, fixed array:
+ *   - The first call on each device looks up the array's address on that device (the device must be the
+ *     current one, as for every call).  Make that first call during start-up, outside any stream capture.
+ *   - All calls on a device use the same array.  Each call clears the part that has to start at zero
+ *     itself (on cuda_stream, before its kernel), so calls issued one after another on one stream are
+ *     safe.  Two calls that can run on the GPU at the same time (different streams without an ordering
+ *     between them, or two host threads) race on the array and give wrong peaks: order them.
+ */
+int fredec_topk_noalloc(const double* z, int64_t K, int32_t k, int64_t* idx_out, int32_t* count_out,
+                        void* cuda_stream);
+int fredec_topk_noalloc_cuda_error(void);        /* the cudaError_t behind its last FREDEC_ECUDA, else 0 */
+int64_t fredec_topk_noalloc_scratch_bytes(void); /* size of the built-in scratch array, per GPU */
 
 /*
  * fredec_scan_topk -- the whole hot path in one call: fredec_scan followed by fredec_topk on

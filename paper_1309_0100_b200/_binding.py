@@ -16,8 +16,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 # FREDEC_LIB: a measurement build of the same library (paper_1309_0100_b200/build.py --variant), for A/B timings
 LIB_PATH = os.environ.get("FREDEC_LIB") or os.path.join(_HERE, "libfredec_b200.so")
 
-FREDEC_OK, FREDEC_EINVAL, FREDEC_EDATA, FREDEC_ESINGULAR, FREDEC_ECUDA = 0, -1, -2, -3, -4
-FREDEC_D_MAX, FREDEC_TOPK_MAX = 64, 1024
+FREDEC_OK, FREDEC_EINVAL, FREDEC_EDATA, FREDEC_ESINGULAR, FREDEC_ECUDA, FREDEC_ELIMIT = 0, -1, -2, -3, -4, -5
+FREDEC_D_MAX, FREDEC_TOPK_MAX, FREDEC_TOPK_NOALLOC_K_MAX = 64, 1024, 128
 
 # name -> (restype, argtypes); must list every symbol include/fredec.h declares
 _P, _I64, _I32, _F64 = C.c_void_p, C.c_int64, C.c_int32, C.c_double
@@ -30,6 +30,9 @@ SIGNATURES = {
     "fredec_chi2_base_batched": (C.c_int, [_P, _P, _P, _I64, _I64, _P, _I32, _P]),
     "fredec_topk": (C.c_int, [_P, _I64, _I32, _P]),
     "fredec_topk_batched": (C.c_int, [_P, _I64, _I64, _I32, _P]),
+    "fredec_topk_noalloc": (C.c_int, [_P, _I64, _I32, _P, _P, _P]),
+    "fredec_topk_noalloc_cuda_error": (C.c_int, []),
+    "fredec_topk_noalloc_scratch_bytes": (C.c_int64, []),
     "fredec_zstat": (C.c_int, [_P, _I64, _F64, _F64, _P]),
     "fredec_fap1": (C.c_int, [_P, _I64, _F64, _F64, _P]),
     "fredec_bandwidth": (C.c_int, [_P, _P, _I64, _F64, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
@@ -223,6 +226,33 @@ def fredec_topk(z, k, idx_out=None):
     pi, ki = _ptr(idx, np.int64)
     count = _check(lib().fredec_topk(pz, K, int(k), pi), "fredec_topk")
     return idx, count
+
+
+def fredec_topk_noalloc(z, k, idx_out, count_out, stream=None):
+    """fredec_topk for callers that may not allocate device memory (include/fredec.h): the library's only
+    scratch is an array built into it, so nothing here or below calls cudaMalloc.  z, idx_out (int64 [k]) and
+    count_out (int32 [1]) are CUDA tensors that the CALLER provides -- this wrapper creates none; stream is
+    None (default stream), an int cudaStream_t or a torch.cuda.Stream.  Returns as soon as the work is
+    enqueued: synchronise with the stream before reading idx_out / count_out.  Calls that may overlap on
+    the GPU race on the shared array; k <= FREDEC_TOPK_NOALLOC_K_MAX."""
+    import torch
+    if not (_is_torch(z) and _is_torch(idx_out) and _is_torch(count_out)):
+        raise TypeError("fredec_topk_noalloc takes caller-provided CUDA tensors only")
+    if count_out.dtype != torch.int32 or count_out.numel() < 1 or not count_out.is_contiguous():
+        raise TypeError("count_out: contiguous int32 tensor with one element")
+    if idx_out.numel() < int(k):
+        raise ValueError("idx_out is shorter than k")
+    pz, kz = _ptr(z)
+    pi, ki = _ptr(idx_out, np.int64)
+    h = 0 if stream is None else int(getattr(stream, "cuda_stream", stream))
+    rc = lib().fredec_topk_noalloc(pz, int(z.shape[-1]), int(k), pi, count_out.data_ptr(), h or None)
+    if rc == FREDEC_ECUDA:
+        raise FredecError(rc, "fredec_topk_noalloc", f"cudaError {lib().fredec_topk_noalloc_cuda_error()}")
+    _check(rc, "fredec_topk_noalloc")
+
+
+def fredec_topk_noalloc_scratch_bytes() -> int:
+    return int(lib().fredec_topk_noalloc_scratch_bytes())
 
 
 def fredec_topk_batched(z, k, idx_out=None):

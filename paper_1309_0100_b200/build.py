@@ -17,7 +17,7 @@ ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 OBJ = os.path.join(PKG, "build")
 LIB = os.path.join(PKG, "libfredec_b200.so")
-SOURCES = ["fredec_api.cu", "prep_kernel.cu", "scan_mma_kernel.cu", "topk_kernel.cu", "peak_kernel.cu", "stat_kernel.cu", "trig_kernel.cu", "subset_kernel.cu", "refine_kernel.cu"]
+SOURCES = ["fredec_api.cu", "prep_kernel.cu", "scan_mma_kernel.cu", "topk_kernel.cu", "topk_noalloc.cu", "peak_kernel.cu", "stat_kernel.cu", "trig_kernel.cu", "subset_kernel.cu", "refine_kernel.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
 

@@ -1088,6 +1088,7 @@ const char* fredec_strerror(int code)
         case FREDEC_EDATA: return "invalid data (non-finite value, negative weight or zero total weight)";
         case FREDEC_ESINGULAR: return "base functions are linearly dependent";
         case FREDEC_ECUDA: return "CUDA error (see fredec_last_cuda_error)";
+        case FREDEC_ELIMIT: return "size exceeds the fixed capacity of a no-allocation entry point";
         default: return code > 0 ? "ok (count)" : "unknown error";
     }
 }

@@ -63,7 +63,7 @@ def test_no_oracle_or_cpu_fallback_in_product():
 def test_strerror_and_version(fr):
     L = fr.lib()
     assert fr.fredec_version() >= 100
-    for code in (0, -1, -2, -3, -4):
+    for code in (0, -1, -2, -3, -4, -5):
         assert len(L.fredec_strerror(code)) > 0
 
 
@@ -83,6 +83,19 @@ def test_argument_validation_needs_no_gpu(fr):
     assert code(lambda: fr.fredec_scan(t, x, w, np.ones((65, 20)), 0.1, 0.1, 5)) == fr.FREDEC_EINVAL
     assert code(lambda: fr.fredec_topk(np.zeros(4), 5)) == fr.FREDEC_EINVAL
     assert code(lambda: fr.fredec_topk(np.zeros(4000), 1025)) == fr.FREDEC_EINVAL
+
+
+def test_noalloc_entry_point_checks_sizes_before_touching_cuda(fr):
+    """fredec_topk_noalloc: argument and capacity errors come back without a GPU (and without a CUDA call)."""
+    L = fr.lib()
+    z = np.zeros(4000); idx = np.zeros(200, dtype=np.int64); cnt = np.zeros(1, dtype=np.int32)
+    pz, pi, pc = z.ctypes.data, idx.ctypes.data, cnt.ctypes.data
+    assert L.fredec_topk_noalloc(pz, 4000, fr.FREDEC_TOPK_NOALLOC_K_MAX + 1, pi, pc, None) == fr.FREDEC_ELIMIT
+    assert L.fredec_topk_noalloc(pz, 4000, 0, pi, pc, None) == fr.FREDEC_EINVAL
+    assert L.fredec_topk_noalloc(pz, 4, 5, pi, pc, None) == fr.FREDEC_EINVAL
+    assert L.fredec_topk_noalloc(None, 4000, 5, pi, pc, None) == fr.FREDEC_EINVAL
+    assert L.fredec_topk_noalloc(pz, 4000, 5, pi, pc, None) in (fr.FREDEC_EINVAL, fr.FREDEC_ECUDA)  # host pointers
+    assert b"capacity" in L.fredec_strerror(fr.FREDEC_ELIMIT)
 
 
 def test_compute_fails_loudly_without_gpu(fr):
