@@ -195,7 +195,9 @@ def run_small_configs(fr, inputs, dev, stream, peak_nominal, with_oracle: bool):
         b.record(stream)
         torch.cuda.synchronize()
         step_ms = a.elapsed_time(b) / steps
-        # the asynchronous form without the per-stage timing events: no host round trip between the steps
+        # the asynchronous form without the per-stage timing events: the host's wait for step n is deferred to the
+        # start of step n + 1 (steps are not pipelined; what is saved is the event records and the idle gap between
+        # return and next call)
         fr.fredec_set_async(True)
         fr.fredec_set_timing(False)
         try:

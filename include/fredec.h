@@ -285,8 +285,8 @@ int fredec_refine(const double* t, const double* x, const double* w, int64_t N,
  *   t, x, w [N];  pool_freqs [n_pool], finite, 1 <= n_pool <= 25: the start frequencies
  *   masks [T]     bit j of masks[i] selects pool_freqs[j] for tuple i (0 <= masks[i] < 2^n_pool; the empty
  *                 tuple is the constant alone); NULL: every tuple is the whole pool.  N >= 3m + 2 for the
- *                 largest tuple size m (host masks are checked; device masks are not read back, and the
- *                 requirement is then N >= 3 n_pool + 2)
+ *                 largest tuple size m.  Host or device; a mask out of range is FREDEC_EINVAL either way
+ *                 (device masks are checked, and m found, by a small kernel before the fits start)
  *   max_iter, tol as fredec_refine
  *   freqs_out [T][n_pool]  refined frequencies of the selected entries, pool_freqs[j] for the others
  *   l_out [T]              min chi2 at the returned frequencies
@@ -311,8 +311,11 @@ int fredec_set_stream(void* cuda_stream);
  * the library's stream, PROVIDED every data pointer of the call is a device pointer (a call with a host
  * pointer stays synchronous: the library may keep no host pointer after return).  Argument errors are
  * still returned at once.  Data errors (FREDEC_EDATA, FREDEC_ESINGULAR) and the peak count are then
- * obtained with fredec_last_status().  The next compute call resolves a pending one first (their status
- * buffers are shared), so at most one call is ever pending.  enable == 0 (default): synchronous.
+ * obtained with fredec_last_status().  The next compute call waits for a pending one before it enqueues
+ * anything (their status buffers are shared), so at most one call is ever pending and consecutive calls are
+ * NOT pipelined: the mode defers the host's wait to the next call, it does not remove it.  If that wait finds
+ * a data error, the error is kept and the next fredec_last_status() reports it (the first such error wins).
+ * enable == 0 (default): synchronous.
  */
 int fredec_set_async(int32_t enable);
 
@@ -320,9 +323,13 @@ int fredec_set_async(int32_t enable);
  * fredec_last_status -- waits for the pending asynchronous call, if any (synchronises the stream), and
  * returns the status the synchronous form would have returned: FREDEC_OK or a negative code; *count_out
  * (may be NULL) receives the number of peaks of series 0 when the call extracted peaks.  Without a
- * pending call it repeats the status of the last resolved one.
+ * pending call it repeats the status of the last resolved one.  An error of an earlier asynchronous call
+ * that a later call had to wait for is reported here first, once.
  */
 int fredec_last_status(int32_t* count_out);
+
+/* 1 while an asynchronous call is enqueued and its status has not been read, else 0. */
+int fredec_pending(void);
 
 /* Device-side durations (ms, CUDA events on the library's stream) of the kernels of the LAST
  * compute call: out[0] = base orthogonalisation + packing kernel(s), out[1] = scan kernel(s),

@@ -47,6 +47,7 @@ SIGNATURES = {
     "fredec_set_async": (C.c_int, [_I32]),
     "fredec_set_timing": (C.c_int, [_I32]),
     "fredec_last_status": (C.c_int, [C.POINTER(C.c_int32)]),
+    "fredec_pending": (C.c_int, []),
     "fredec_last_timing": (C.c_int, [C.POINTER(C.c_double)]),
     "fredec_last_launches": (C.c_int, []),
     "fredec_bench_fp64": (C.c_int, [_I32, _I64, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
@@ -167,7 +168,8 @@ def fredec_scan_batched(t, x, w, base_funcs, f0, df, K, z_out=None):
 
 
 def fredec_scan_topk(t, x, w, base_funcs, f0, df, K, k, z_out=None, idx_out=None, want_z=True):
-    """Scan + peaks in one call.  Returns (z or None, idx[k], count)."""
+    """Scan + peaks in one call.  Returns (z or None, idx[k], count); count is None when the call was only
+    enqueued (fredec_set_async): fredec_last_status() then delivers it."""
     N = int(t.shape[-1])
     d = 0 if base_funcs is None else int(base_funcs.shape[0])
     if d == 0:
@@ -178,7 +180,7 @@ def fredec_scan_topk(t, x, w, base_funcs, f0, df, K, k, z_out=None, idx_out=None
     pi, ki = _ptr(idx, np.int64)
     count = _check(lib().fredec_scan_topk(pt, px, pw, N, pb, d, float(f0), float(df), int(K), pz,
                                           int(k), pi), "fredec_scan_topk")
-    return z, idx, count
+    return z, idx, (None if lib().fredec_pending() else count)   # asynchronous: the count is fredec_last_status()
 
 
 def fredec_scan_topk_batched(t, x, w, base_funcs, f0, df, K, k, z_out=None, idx_out=None, want_z=True):
@@ -225,7 +227,7 @@ def fredec_topk(z, k, idx_out=None):
     pz, kz = _ptr(z)
     pi, ki = _ptr(idx, np.int64)
     count = _check(lib().fredec_topk(pz, K, int(k), pi), "fredec_topk")
-    return idx, count
+    return idx, (None if lib().fredec_pending() else count)      # asynchronous: the count is fredec_last_status()
 
 
 def fredec_topk_noalloc(z, k, idx_out, count_out, stream=None):
@@ -344,15 +346,20 @@ def fredec_refine_batched(t, x, w, pool_freqs, masks=None, max_iter=20, tol=1e-9
     masks=None with T: T copies of the whole pool).  Returns (freqs [T][n_pool], l [T], iters [T] int32,
     status [T] int32) as numpy arrays."""
     N, n_pool = int(t.shape[-1]), int(pool_freqs.shape[-1])
-    if masks is not None:
+    pm = None
+    if masks is not None and _is_torch(masks) and masks.is_cuda:
+        pm, km = _ptr(masks, np.int64)                       # device masks: used in place
+        T = int(masks.shape[0])
+    elif masks is not None:
         masks = np.ascontiguousarray(masks.cpu().numpy() if _is_torch(masks) else masks, dtype=np.int64)
         T = int(masks.shape[0])
+        pm = masks.ctypes.data
     T = 1 if T is None else int(T)
     freqs = np.empty((T, n_pool))
     l = np.empty(T)
     iters, status = np.empty(T, dtype=np.int32), np.empty(T, dtype=np.int32)
     (pt, kt), (px, kx), (pw, kw), (pp, kp) = map(_ptr, (t, x, w, pool_freqs))
-    _check(lib().fredec_refine_batched(pt, px, pw, N, pp, n_pool, None if masks is None else masks.ctypes.data, T,
+    _check(lib().fredec_refine_batched(pt, px, pw, N, pp, n_pool, pm, T,
                                        int(max_iter), float(tol), freqs.ctypes.data, l.ctypes.data,
                                        iters.ctypes.data, status.ctypes.data), "fredec_refine_batched")
     return freqs, l, iters, status

@@ -95,6 +95,7 @@ struct State {
     bool pend_series = false, pend_topk = false;
     int64_t pend_B = 0;
     int last_status = 0, last_count = 0;
+    int unread_status = 0;  // first error of a pending call that was settled by a later call, not yet reported
     // the per-stage timing events of the scan / top-k calls; off inside fredec_phase1, whose iterations are
     // short enough for seven event records each to show
     bool timing_on = true;
@@ -229,12 +230,13 @@ struct Call {
 };
 
 int resolve_pending();
+void settle_pending();
 
 int begin_call()
 {
     int rc = ensure_ready();
     if (rc) return rc;
-    if (g.pending) (void)resolve_pending();  // its events and pinned status buffers are about to be reused
+    settle_pending();  // its events and pinned status buffers are about to be reused
     g.launches = 0;
     for (double& v : g.timing) v = 0.0;
     CK(record_event(0));
@@ -497,6 +499,15 @@ int resolve_pending()
     return g.last_status;
 }
 
+// A pending call that something other than fredec_last_status has to wait for: its error, if any, is kept
+// for the next fredec_last_status instead of being lost.
+void settle_pending()
+{
+    if (!g.pending) return;
+    const int rc = resolve_pending();
+    if (rc < 0 && g.unread_status == 0) g.unread_status = rc;
+}
+
 // Copies results out and either synchronises and reads the statuses (*first_count = peaks of series 0),
 // or -- `defer`, or the asynchronous mode with nothing to copy to the host -- leaves the call pending.
 int finish_call(Call& c, int* first_count, bool defer = false)
@@ -578,6 +589,9 @@ int do_chi2(const double* t, const double* x, const double* w, int64_t B, int64_
     Call c;
     if ((rc = enqueue_series(c, t, x, w, B, N, base_funcs, d, 0.0, 1.0, 1, nullptr, false))) return rc;
     if ((rc = finish_call(c, nullptr))) return rc;
+    // chi2 is read from the pinned status records below: in the asynchronous mode finish_call may have left
+    // the call pending (fredec.h: only the scan / top-k calls are asynchronous), so wait for it here
+    if (g.pending && (rc = resolve_pending())) return rc;
     const SeriesInfo* hi = static_cast<const SeriesInfo*>(g.h_info.p);
     if (on_device(chi2_out)) {
         double* tmp = static_cast<double*>(std::malloc((size_t)B * 8));
@@ -915,8 +929,8 @@ int fredec_refine_batched(const double* t, const double* x, const double* w, int
     int rc = begin_call();
     if (rc) return rc;
     cudaStream_t st = g.stream;
-    // the largest tuple sizes the shared memory and the N >= 3m + 2 requirement; masks on the device are
-    // not read back: the whole pool is then the bound
+    // the largest tuple sizes the shared memory (hence the CTAs resident per SM) and the N >= 3m + 2
+    // requirement; masks on the device are measured by a small kernel whose two counters are read back
     int m_max = n_pool;
     if (masks && !on_device(masks)) {
         m_max = 0;
@@ -926,6 +940,16 @@ int fredec_refine_batched(const double* t, const double* x, const double* w, int
             for (int j = 0; j < n_pool; ++j) c += (int)((masks[i] >> j) & 1);
             m_max = c > m_max ? c : m_max;
         }
+    } else if (masks) {
+        int stats[2] = {0, 0};
+        CK(g.sink.reserve(64));
+        int* dstats = reinterpret_cast<int*>(g.sink.as<double>() + 6);  // bytes 48..55; bandwidth uses 0..31
+        CK(launch_mask_stats(masks, T, n_pool, dstats, st));
+        CK(cudaMemcpyAsync(stats, dstats, sizeof(stats), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        g.launches += 1;
+        if (stats[1] != 0) return FREDEC_EINVAL;
+        m_max = stats[0];
     }
     if (N < 3 * (int64_t)m_max + 2) return FREDEC_EINVAL;
     const double *dt, *dx, *dw, *dpool;
@@ -993,35 +1017,42 @@ int fredec_refine(const double* t, const double* x, const double* w, int64_t N, 
 
 int fredec_set_stream(void* cuda_stream)
 {
+    settle_pending();  // the pending call was enqueued on the old stream: wait on that one
     g.stream = static_cast<cudaStream_t>(cuda_stream);
     return FREDEC_OK;
 }
 
 int fredec_set_async(int32_t enable)
 {
-    if (g.pending) (void)resolve_pending();
+    settle_pending();
     g.async_mode = enable != 0;
     return FREDEC_OK;
 }
 
 int fredec_last_status(int32_t* count_out)
 {
-    const int rc = resolve_pending();
+    int rc = resolve_pending();
+    if (g.unread_status != 0) {  // an earlier asynchronous call failed and nobody has been told yet
+        rc = g.unread_status;
+        g.unread_status = 0;
+    }
     if (count_out) *count_out = rc == FREDEC_OK ? g.last_count : 0;
     return rc;
 }
 
+int fredec_pending(void) { return g.pending ? 1 : 0; }
+
 int fredec_last_timing(double out[4])
 {
     if (!out) return FREDEC_EINVAL;
-    if (g.pending) (void)resolve_pending();
+    settle_pending();
     for (int i = 0; i < 4; ++i) out[i] = g.timing[i];
     return FREDEC_OK;
 }
 
 int fredec_set_timing(int32_t enable)
 {
-    if (g.pending) (void)resolve_pending();
+    settle_pending();
     g.timing_on = enable != 0;
     return FREDEC_OK;
 }
@@ -1065,6 +1096,7 @@ const char* fredec_bench_fp64_name(int32_t mode)
 
 int fredec_shutdown(void)
 {
+    settle_pending();  // it reads the pinned status buffers released below
     DevBuf* bufs[] = {&g.fz, &g.fi, &g.fedge, &g.fthr, &g.in_t, &g.in_x, &g.in_w, &g.in_base, &g.in_z, &g.out_z, &g.out_idx, &g.out_chi2, &g.gram, &g.rf, &g.part, &g.p1_base, &g.p1_freq, &g.p1_z, &g.p1_idx, &g.p1_stats, &g.tab, &g.srec,
                       &g.psi,  &g.xt,   &g.info, &g.ws, &g.red,     &g.part_z, &g.part_i, &g.count, &g.sink};
     for (DevBuf* b : bufs) b->release();
@@ -1076,6 +1108,10 @@ int fredec_shutdown(void)
     if (g.ready)
         for (int i = 0; i < kNumEvents; ++i) cudaEventDestroy(g.ev[i]);
     g.ready = false;
+    g.pending = g.pend_series = g.pend_topk = false;
+    g.last_status = FREDEC_OK;
+    g.last_count = 0;
+    g.unread_status = 0;
     (void)cudaGetLastError();
     return FREDEC_OK;
 }

@@ -263,7 +263,37 @@ __global__ void __launch_bounds__(kRefThreads) refine_batched_kernel(RefineParam
     if (tid < m) p.freqs_out[tuple * p.n_pool + sel[tid]] = f[tid];
 }
 
+// out[0] = largest number of selected frequencies of any tuple, out[1] = number of masks that are negative
+// or select an entry beyond the pool (both start at zero)
+__global__ void mask_stats_kernel(const int64_t* __restrict__ masks, int64_t T, int n_pool, int* __restrict__ out)
+{
+    int m = 0, bad = 0;
+    const int64_t limit = (int64_t)1 << n_pool;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < T; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t mk = masks[i];
+        if (mk < 0 || mk >= limit) ++bad;
+        else m = max(m, __popcll((unsigned long long)mk));
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
+        bad += __shfl_xor_sync(0xffffffffu, bad, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        if (m > 0) atomicMax(out, m);
+        if (bad > 0) atomicAdd(out + 1, bad);
+    }
+}
+
 }  // namespace
+
+cudaError_t launch_mask_stats(const int64_t* masks, int64_t T, int n_pool, int* out2, cudaStream_t stream)
+{
+    cudaError_t e = cudaMemsetAsync(out2, 0, 2 * sizeof(int), stream);
+    if (e != cudaSuccess) return e;
+    const int64_t blocks = (T + 255) / 256;
+    mask_stats_kernel<<<(unsigned)(blocks < 592 ? blocks : 592), 256, 0, stream>>>(masks, T, n_pool, out2);
+    return cudaGetLastError();
+}
 
 size_t refine_batched_smem(int m_max) { return ref_smem(m_max).total; }
 

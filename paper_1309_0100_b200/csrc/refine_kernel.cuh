@@ -30,5 +30,8 @@ struct RefineParams {
 // clamped to +-0.5 / T_eff (reading R1) -> stop when max |step| T_eff <= tol (reading R2).
 cudaError_t launch_refine_batched(const RefineParams& p, int64_t T, int m_max, cudaStream_t stream);
 size_t refine_batched_smem(int m_max);
+// Tuple masks that live on the device: out2[0] = the largest tuple size, out2[1] = how many masks are out of
+// range (negative, or a bit at or beyond n_pool).  out2: two ints of device memory.
+cudaError_t launch_mask_stats(const int64_t* masks, int64_t T, int n_pool, int* out2, cudaStream_t stream);
 
 }  // namespace fredec

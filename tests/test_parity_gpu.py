@@ -106,6 +106,47 @@ def test_config4_full_size_sampled(fr, oracle_mod):
     assert np.max(np.abs(z_slice - z[k1:k1 + n])) <= RTOL_MAXZ * zmax
 
 
+@pytest.mark.slow
+def test_config4_full_size_every_grid_point(fr, oracle_mod):
+    """Config 4 in full, element by element: all 2 000 000 grid points of the launch bench.py times against
+    the oracle on all host cores (every point of the "dense enough" grid is a result), and
+    the peaks END TO END: fredec_topk of the GPU periodogram == oracle_topk of the ORACLE periodogram."""
+    wl = inputs.config(4)
+    t, x, w, base = wl.series(0)
+    dt, dx, dw, db = _dev(t, x, w, base)
+    z_dev = fr.fredec_scan(dt, dx, dw, db, wl.f0, wl.df, wl.K)
+    idx_gpu, cnt = fr.fredec_topk(z_dev, wl.topk)
+    z_ref = oracle_mod.scan(t, x, w, base, wl.f0, wl.df, wl.K, threads=0)
+    assert_parity(z_dev.cpu().numpy(), z_ref, wl.name)
+    idx_ref, cnt_ref = oracle_mod.topk(z_ref, wl.topk)
+    assert cnt == cnt_ref and idx_gpu.cpu().numpy().tolist() == idx_ref.tolist()
+
+
+@pytest.mark.slow
+def test_config5_full_size_256_whole_series_and_all_peaks(fr, oracle_mod):
+    """Config 5 as bench.py launches it (4096 x 500 x 100 000).  256 series spread over the batch are compared
+    with the oracle on every grid point, peaks end to end (GPU peaks of GPU z == oracle peaks of oracle z);
+    for ALL 4096 series the GPU's indices equal the oracle's peak finder on the GPU's periodogram, and the
+    fused path (no periodogram) gives the same indices."""
+    wl = inputs.config(5)
+    dt, dx, dw, db = _dev(wl.t, wl.x, wl.w, wl.base_funcs)
+    z, idx = fr.fredec_scan_topk_batched(dt, dx, dw, db, wl.f0, wl.df, wl.K, wl.topk)
+    idx = idx.cpu().numpy()
+    whole = set(np.linspace(0, wl.B - 1, 256).astype(int).tolist())
+    worst = 0.0
+    for b in range(wl.B):
+        zb = z[b].cpu().numpy()
+        assert idx[b].tolist() == oracle_mod.topk(zb, wl.topk)[0].tolist(), f"series {b}"
+        if b in whole:
+            t, x, w, base = wl.series(b)
+            z_ref = oracle_mod.scan(t, x, w, base, wl.f0, wl.df, wl.K, threads=0)
+            worst = max(worst, assert_parity(zb, z_ref, f"series {b}"))
+            assert idx[b].tolist() == oracle_mod.topk(z_ref, wl.topk)[0].tolist(), f"series {b} end to end"
+    del z
+    _, idx_f = fr.fredec_scan_topk_batched(dt, dx, dw, db, wl.f0, wl.df, wl.K, wl.topk, want_z=False)
+    assert np.array_equal(idx_f.cpu().numpy(), idx)
+
+
 # ------------------------------------------------------------------ config 5 (batched)
 def test_config5_reduced_batch_full_parity(fr, oracle_mod):
     wl = inputs.config(5, B=12, K=20_000)
@@ -306,7 +347,7 @@ def test_asynchronous_form(fr, oracle_mod):
         z = torch.empty(wl.K, dtype=torch.float64, device="cuda")
         idx = torch.empty(10, dtype=torch.int64, device="cuda")
         _, _, rc = fr.fredec_scan_topk(dt, dx, dw, db, wl.f0, wl.df, wl.K, 10, z_out=z, idx_out=idx)
-        assert rc == 0                                     # enqueued: the count comes from last_status
+        assert rc is None                                  # enqueued: the count comes from last_status
         assert fr.fredec_last_status() == cnt_sync
         torch.cuda.synchronize()
         assert torch.equal(z, z_sync) and torch.equal(idx, idx_sync)
@@ -320,12 +361,61 @@ def test_asynchronous_form(fr, oracle_mod):
         with pytest.raises(fr.FredecError) as e:
             fr.fredec_last_status()
         assert e.value.code == fr.FREDEC_EDATA
+        # an error that the NEXT call has to wait for is not lost: last_status reports it once
+        fr.fredec_scan(dt, bad, dw, db, wl.f0, wl.df, wl.K)
+        fr.fredec_scan(dt, dx, dw, db, wl.f0, wl.df, wl.K)
+        with pytest.raises(fr.FredecError) as e:
+            fr.fredec_last_status()
+        assert e.value.code == fr.FREDEC_EDATA
+        assert fr.fredec_last_status() == 0
         # host pointers: synchronous as ever
         zh, idxh, cnth = fr.fredec_scan_topk(t, x, w, base, wl.f0, wl.df, wl.K, 10)
         assert cnth == cnt_sync and np.array_equal(zh, z_sync.cpu().numpy())
     finally:
         fr.fredec_set_async(False)
     assert fr.fredec_scan_topk(dt, dx, dw, db, wl.f0, wl.df, wl.K, 10)[2] == cnt_sync
+
+
+def test_async_mode_chi2_stream_switch_and_shutdown(fr):
+    """Three corners of the asynchronous mode: fredec_chi2_base stays synchronous (it reads the status
+    records on the host) and reports data errors; fredec_set_stream and fredec_shutdown settle a pending
+    call first instead of waiting on the wrong stream / reading released buffers."""
+    import torch
+    wl = inputs.config(2, K=20_000)
+    t, x, w, base = wl.series(0)
+    dt, dx, dw, db = _dev(t, x, w, base)
+    chi2_sync = fr.fredec_chi2_base(dt, dx, dw, db)
+    z_sync = fr.fredec_scan(dt, dx, dw, db, wl.f0, wl.df, wl.K)
+    fr.fredec_set_async(True)
+    try:
+        # an earlier call with another chi2 in the status records, then chi2 in async mode
+        fr.fredec_chi2_base(dt, 3.0 * dx, dw, db)
+        assert fr.fredec_chi2_base(dt, dx, dw, db) == chi2_sync
+        bad = dx.clone(); bad[3] = float("inf")
+        with pytest.raises(fr.FredecError) as e:
+            fr.fredec_chi2_base(dt, bad, dw, db)
+        assert e.value.code == fr.FREDEC_EDATA
+        # pending call, then a stream switch: the status must be that call's
+        s = torch.cuda.Stream()
+        z = fr.fredec_scan(dt, dx, dw, db, wl.f0, wl.df, wl.K)
+        fr.fredec_set_stream(s)
+        assert fr.fredec_last_status() == 0
+        assert torch.equal(z, z_sync)                      # resolved: complete without a further sync
+        s.wait_stream(torch.cuda.current_stream())
+        z = fr.fredec_scan(dt, dx, dw, db, wl.f0, wl.df, wl.K)
+        fr.fredec_set_stream(None)
+        assert torch.equal(z, z_sync)
+        # pending call, then shutdown, then more calls
+        z = fr.fredec_scan(dt, dx, dw, db, wl.f0, wl.df, wl.K)
+        fr.fredec_shutdown()
+        assert torch.equal(z, z_sync)
+        assert fr.fredec_last_status() == 0
+        z = fr.fredec_scan(dt, dx, dw, db, wl.f0, wl.df, wl.K)
+        assert fr.fredec_last_status() == 0 and torch.equal(z, z_sync)
+    finally:
+        fr.fredec_set_stream(None)
+        fr.fredec_set_async(False)
+    assert fr.fredec_chi2_base(dt, dx, dw, db) == chi2_sync
 
 
 def test_stage_timing_switch(fr):
@@ -385,15 +475,14 @@ def test_singular_trial_frequency(fr, oracle_mod):
     assert abs(z[0] - np.sum(w * x) ** 2 / np.sum(w)) <= 1e-12 * np.sum(w * x * x)
 
 
-def test_near_singular_band_rule_s6(fr, oracle_mod):
+def test_near_singular_band_rule_s6(fr, oracle_mod, report):
     """Rule S6: trial frequencies closing in on a base frequency, at
     10^-1 ... 10^-8 cycles over the time span.  Far from the base frequency (relative Schur pivot
     >= 1e-6) the 1e-9 max z tolerance holds; inside the band the two sides lose digits at
     different rates (the oracle in a (d+2)^2 Cholesky of raw functions, the kernel in a Schur
     complement of orthonormalised ones) and may drop the column at slightly different offsets:
-    the disagreement is recorded in gpurun_out/s6_band.txt and bounded by the z of the dropped
+    the disagreement is handed to the `report` fixture (table s6_band) and bounded by the z of the dropped
     column; z stays finite, >= 0 and <= chi2_base everywhere."""
-    import os
     t, x, w, _ = inputs.random_series(606, 400, 0, t_span=200.0)
     T = t.max() - t.min()
     fb = 0.1234
@@ -412,9 +501,8 @@ def test_near_singular_band_rule_s6(fr, oracle_mod):
         else:                 # inside / near the band: bounded by the contribution of the doubtful column
             assert abs(zg - zo) <= max(zg, zo) + 1e-9 * zmax
     assert worst_far <= RTOL_MAXZ * zmax
-    os.makedirs("gpurun_out", exist_ok=True)
-    with open(os.path.join("gpurun_out", "s6_band.txt"), "w") as fh:
-        fh.write("\n".join(lines) + "\n")
+    for line in lines:
+        report("s6_band", line)
 
 
 def test_error_codes(fr):

@@ -207,7 +207,7 @@ def _alias_example_series():
 
 
 @pytest.mark.parametrize("which", ["rv_like_pool", "alias_comb", "near_duplicates"])
-def test_subset_fits_aliased_pools(fr, p1, which):
+def test_subset_fits_aliased_pools(fr, p1, which, report):
     """Pools as phase 1 really produces them ("will likely contain some aliases"): Q of a
     subset that holds a frequency and its aliases is badly conditioned, which is where the walk's
     incrementally updated L^{-1} loses digits.  Pools: (a) the pool the ORACLE's phase 1 finds on the
@@ -217,8 +217,8 @@ def test_subset_fits_aliased_pools(fr, p1, which):
     for the oracle itself to be that accurate (smallest relative pivot >= 1e-4; measured against 40-digit
     arithmetic the FP64 oracle is off by up to 1.7e-5 D on the full comb, whose Q has condition 3e16).
     Below that both sides lose eps / pivot of D: bound 1e3 eps D / pivot down to pivot 1e-8; inside the
-    S6 band only validity (finite, 0 <= l <= l of the constant alone).  The worst cases per class are
-    written to gpurun_out/subset_alias_*.txt."""
+    S6 band only validity (finite, 0 <= l <= l of the constant alone).  The worst cases per class go to
+    the `report` fixture (tables subset_alias_*)."""
     rng = np.random.Generator(np.random.PCG64(7))
     if which == "rv_like_pool":
         wl = inputs.config(2)
@@ -243,13 +243,11 @@ def test_subset_fits_aliased_pools(fr, p1, which):
     err = np.abs(got[masks] - ref)
     well = pmin >= 1e-4                       # class A: the oracle itself is good to ~1e-12 D
     band = (pmin >= 1e-8) & ~well             # class B: eps / pivot of D is lost on either side
-    import os
-    os.makedirs("gpurun_out", exist_ok=True)
-    with open(os.path.join("gpurun_out", f"subset_alias_{which}.txt"), "w") as fh:
-        for name, sel in (("pivot>=1e-4", well), ("1e-8<=pivot<1e-4", band), ("pivot<1e-8 or dropped", ~well & ~band)):
-            if sel.any():
-                fh.write(f"n={n} {name}: masks={int(sel.sum())} max|dl|/D={err[sel].max() / D:.3e} "
-                         f"max|dl|*pivot/(eps D)={np.max(err[sel] * np.maximum(pmin[sel], 1e-300)) / (2.2e-16 * D):.3e}\n")
+    for name, sel in (("pivot>=1e-4", well), ("1e-8<=pivot<1e-4", band), ("pivot<1e-8 or dropped", ~well & ~band)):
+        if sel.any():
+            report(f"subset_alias_{which}",
+                   f"n={n} {name}: masks={int(sel.sum())} max|dl|/D={err[sel].max() / D:.3e} "
+                   f"max|dl|*pivot/(eps D)={np.max(err[sel] * np.maximum(pmin[sel], 1e-300)) / (2.2e-16 * D):.3e}")
     assert np.all(np.isfinite(got)) and np.all(got >= 0.0) and np.all(got <= got[0] * (1 + 1e-12))
     assert well.sum() >= masks.size // 8
     assert err[well].max() <= 1e-10 * D, f"max |dl| / D = {err[well].max() / D:.3e}"
@@ -301,7 +299,7 @@ def test_refine_parity(fr, p1, noise, n):
     assert it0 == 0 and np.array_equal(f0, start) and abs(l0 - l0_ref) <= 1e-9 * D
 
 
-def test_refine_batched_parity_1000_tuples(fr, p1, oracle_mod):
+def test_refine_batched_parity_1000_tuples(fr, p1, oracle_mod, report):
     """PAPER.md:214 / :266: the local fits l_{m,loc} of many subsets of one pool in one call (one CTA per
     tuple, every iteration on the device) against the oracle's refine() looped over the tuples.  Pool: 12
     frequencies near 12 sinusoids of the series (start values up to 0.2 / T off); 1000 random subsets of
@@ -349,15 +347,11 @@ def test_refine_batched_parity_1000_tuples(fr, p1, oracle_mod):
     fd, ld, _, _ = fr.fredec_refine_batched(*[torch.from_numpy(a).cuda() for a in (t, x, w, pool)], masks[:50],
                                              max_iter=30, tol=tol)
     assert np.array_equal(fd, freqs[:50]) and np.array_equal(ld, l[:50])
-    os.makedirs("gpurun_out", exist_ok=True)
-    with open("gpurun_out/refine_batched.txt", "w") as fh:
-        tm = fr.fredec_last_timing()
-        fh.write(f"tuples=50 kernel_ms={tm['scan_ms']:.3f}\n")
+    report("refine_batched", f"tuples=50 kernel_ms={fr.fredec_last_timing()['scan_ms']:.3f}")
     fr.fredec_refine_batched(t, x, w, pool, masks, max_iter=30, tol=tol)
-    with open("gpurun_out/refine_batched.txt", "a") as fh:
-        tm = fr.fredec_last_timing()
-        fh.write(f"tuples={masks.size} N={N} sizes 1..6 (+ empty, full 12): kernel_ms={tm['scan_ms']:.3f} "
-                 f"tuples_per_s={masks.size / (tm['scan_ms'] * 1e-3):.3e}\n")
+    tm = fr.fredec_last_timing()
+    report("refine_batched", f"tuples={masks.size} N={N} sizes 1..6 (+ empty, full 12): kernel_ms={tm['scan_ms']:.3f} "
+                             f"tuples_per_s={masks.size / (tm['scan_ms'] * 1e-3):.3e}")
 
 
 def test_refine_batched_singular_tuple_and_errors(fr):
@@ -371,6 +365,26 @@ def test_refine_batched_singular_tuple_and_errors(fr):
         fr.fredec_refine_batched(t[:10], x[:10], w[:10], pool, np.array([7]))    # N < 3 m + 2
     with pytest.raises(fr.FredecError):
         fr.fredec_refine_batched(t, x, w, np.linspace(0.1, 0.9, 26))           # pool > 25
+
+
+def test_refine_batched_device_masks(fr):
+    """Masks in device memory are measured and range-checked by a small kernel: same fits as host masks, a bit
+    beyond the pool is FREDEC_EINVAL, and N only has to cover the largest tuple actually present."""
+    import torch
+    t, x, w, _ = inputs.random_series(2, 40, 0)
+    pool = np.linspace(0.11, 0.47, 20)                       # N = 40 < 3 * 20 + 2: only small tuples fit
+    masks = np.array([0b11, 0b101, 1 << 19, 0, 0b1110000], dtype=np.int64)
+    ref = fr.fredec_refine_batched(t, x, w, pool, masks)
+    dev = fr.fredec_refine_batched(t, x, w, pool, torch.from_numpy(masks).cuda())
+    for a, b in zip(ref, dev):
+        assert np.array_equal(a, b)
+    for bad in ([0b11, 1 << 20], [-1, 0b11]):
+        with pytest.raises(fr.FredecError) as e:
+            fr.fredec_refine_batched(t, x, w, pool, torch.tensor(bad, dtype=torch.int64, device="cuda"))
+        assert e.value.code == fr.FREDEC_EINVAL
+    with pytest.raises(fr.FredecError) as e:                 # a tuple of 13 needs N >= 41
+        fr.fredec_refine_batched(t, x, w, pool, torch.tensor([(1 << 13) - 1], dtype=torch.int64, device="cuda"))
+    assert e.value.code == fr.FREDEC_EINVAL
 
 
 def test_non_finite_frequencies_are_data_errors(fr):
