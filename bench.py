@@ -242,27 +242,37 @@ def run_small_configs(fr, inputs, dev, stream, peak_nominal, with_oracle: bool):
 def run_phase1(fr, inputs, dev, with_oracle: bool):
     """What the scan is for: phase 1 on the RV-like series of config 2 -- residual
     periodograms with a growing base (d = 1, 3, 5, ...), peaks, statistic and FAP per iteration -- through
-    `fredec_phase1` (device-resident series, one host round trip per iteration), and the oracle's phase 1 on
-    the same arrays: identical pool and base, wall-clock of both."""
+    `fredec_phase1_refined` (device-resident series; after every addition the base frequencies are refitted by
+    the device Gauss-Newton), and the oracle's phase 1 in the same mode on the same arrays:
+    identical pool and base, wall-clock of both.  `grid_only` is `fredec_phase1` (the peak's grid frequency
+    joins the base as it is): more periodograms, because a mis-tuned base leaves a residue that comes back."""
     import torch
     wl = inputs.config(2)
     t, x, w, _ = wl.series(0)
     d_in = [torch.from_numpy(a).to(dev) for a in (t, x, w)]
     kw = dict(fap0=0.05, fap1=0.1, A1=1.0, max_base=12, k_peaks=32)
-    res = fr.fredec_phase1(*d_in, wl.f0, wl.df, wl.K, **kw)           # warm-up
-    torch.cuda.synchronize()
-    t0 = time.perf_counter()
-    res = fr.fredec_phase1(*d_in, wl.f0, wl.df, wl.K, **kw)
-    torch.cuda.synchronize()
-    ms = 1e3 * (time.perf_counter() - t0)
-    n_it = int(res["base_idx"].size) + 1                               # the last periodogram stops the loop
-    rec = {"workload": f"phase 1 on {wl.name}: N={wl.N} x K={wl.K}, base grows to d={2 * res['base_idx'].size + 1}",
-           "ms": ms, "periodograms": n_it, "launches": fr.fredec_last_launches(),
-           "pool_size": int(res["pool_idx"].size), "base_idx": res["base_idx"].tolist()}
+
+    def timed(**mode):
+        fr.fredec_phase1(*d_in, wl.f0, wl.df, wl.K, **kw, **mode)     # warm-up
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        res = fr.fredec_phase1(*d_in, wl.f0, wl.df, wl.K, **kw, **mode)
+        torch.cuda.synchronize()
+        ms = 1e3 * (time.perf_counter() - t0)
+        n_it = int(res["base_idx"].size) + 1                           # the last periodogram stops the loop
+        return res, {"ms": ms, "periodograms": n_it, "launches": fr.fredec_last_launches(),
+                     "pool_size": int(res["pool_idx"].size), "base_idx": res["base_idx"].tolist()}
+
+    res, rec = timed(refine_base=True, refine_iter=30, refine_tol=1e-11)
+    rec = {"workload": f"phase 1 on {wl.name}: N={wl.N} x K={wl.K}, base refitted after every addition, grows to "
+                       f"d={2 * res['base_idx'].size + 1}", **rec,
+           "base_periods": [round(1.0 / f, 4) for f in res["base_freqs"].tolist()]}
+    rec["grid_only"] = timed()[1]
     if with_oracle:
         from oracle import phase1 as p1
         t0 = time.perf_counter()
-        ref = p1.phase1(t, x, w, wl.f0, wl.df, wl.K, fap0=0.05, fap1_thr=0.1, A1=1.0, max_base=12, k_peaks=32, threads=0)
+        ref = p1.phase1(t, x, w, wl.f0, wl.df, wl.K, fap0=0.05, fap1_thr=0.1, A1=1.0, max_base=12, k_peaks=32,
+                        threads=0, refine_base=True, refine_iter=30, refine_tol=1e-11)
         rec["oracle_ms"] = 1e3 * (time.perf_counter() - t0)
         rec["pool_equal_oracle"] = (res["pool_idx"].tolist() == ref["pool_idx"].tolist()
                                     and res["base_idx"].tolist() == ref["base_idx"].tolist())
@@ -441,6 +451,20 @@ def main_ours(args):
                  "topk": {"bound": "hbm", "achieved": zbytes / (best["topk_ms"] * 1e-3) / 1e9, "peak": hbm_peak,
                           "unit": "GB/s", "frac": zbytes / (best["topk_ms"] * 1e-3) / 1e9 / hbm_peak,
                           "peak_source": "MEASURED_PEAKS.json hbm_gbs (copy), else 6551.4"}}
+        if cpu is not None:
+            # the oracle on the first 8 series of config 5 (every grid point), one core and all cores
+            import oracle
+            rates = {}
+            for label, threads in (("all_cores", 0), ("one_core", 1)):
+                nser = 8 if threads == 0 else 2
+                t0 = time.perf_counter()
+                for b in range(nser):
+                    oracle.topk(oracle.scan(*wl5.series(b), wl5.f0, wl5.df, wl5.K, threads=threads), wl5.topk)
+                rates[label] = nser * wl5.N * wl5.K / (time.perf_counter() - t0) / 1e9
+            multi["cpu_baseline"] = {"value": rates["all_cores"], "unit": "Gpairs/s", "cores": oracle.num_threads(),
+                                     "kind": "oracle", "one_core_gpairs_s": rates["one_core"],
+                                     "sample": "first 8 of 4096 series of config 5, all 100000 grid frequencies each "
+                                               "(one core: first 2 series)"}
         del d5, z5, i5
 
     sm_count = torch.cuda.get_device_properties(dev).multi_processor_count

@@ -213,8 +213,8 @@ int fredec_bandwidth(const double* t, const double* w, int64_t N, double f_max, 
  *   height >= half of the highest goes to the pool (a grid point already in the
  *   pool keeps its smaller FAP), and the highest peak's frequency joins the base.
  *   Finally the pool is cut to N/10 entries of smallest FAP.
- * This build adds the GRID frequency of the peak to the base (no non-linear refinement, which is
- * SURVEY 8(f) NEXT-3); DESIGN.md section 11 lists the readings.
+ * fredec_phase1 adds the GRID frequency of the peak to the base; fredec_phase1_refined (below) refits the
+ * base frequencies after every addition.  DESIGN.md section 11 lists the readings.
  *
  *   t, x, w [N], f0, df, K        as fredec_scan (the base model is built internally)
  *   fap0 <= fap1 in (0, 1]        thresholds (PAPER.md:228 defaults: 0.05 and 0.1);  A1 as fredec_fap1
@@ -232,6 +232,28 @@ int fredec_phase1(const double* t, const double* x, const double* w, int64_t N,
                   double fap0, double fap1, double A1, int32_t max_base, int32_t k_peaks,
                   int64_t* pool_idx, double* pool_z, double* pool_fap, int32_t pool_cap,
                   int64_t* base_idx, int32_t* n_base_out);
+
+/*
+ * fredec_phase1_refined -- phase 1 with the base model fitted as the paper fits such models: after the
+ * grid frequency of the highest peak has joined the base, ALL base frequencies are refitted
+ * together by the local multifrequency fit of PAPER.md:177-185 (eq. 17; the device Gauss-Newton of
+ * fredec_refine, started from the current values), and the next residual periodogram is computed against
+ * constant + sinusoids at the refitted, off-grid frequencies (reading P5).  A signal
+ * up to df/2 away from the nearest grid point is then removed whole, instead of leaving a residue that
+ * re-enters the base and the pool at the neighbouring grid point a few iterations later.
+ *   refine_iter >= 0, refine_tol > 0   as max_iter, tol of fredec_refine (20 and 1e-9 are sensible)
+ *   max_base <= 25                     (the limit of fredec_refine)
+ *   base_idx [max_base]                HOST: grid index of each iteration's highest peak, in the order found
+ *   base_freq [max_base]               HOST: the frequencies the base model ends with (refitted)
+ * Everything else as fredec_phase1, including the pool (grid indices of periodogram peaks).  If a refit
+ * fails (singular normal equations) that iteration keeps its unrefined frequencies.
+ */
+int fredec_phase1_refined(const double* t, const double* x, const double* w, int64_t N,
+                          double f0, double df, int64_t K,
+                          double fap0, double fap1, double A1, int32_t max_base, int32_t k_peaks,
+                          int32_t refine_iter, double refine_tol,
+                          int64_t* pool_idx, double* pool_z, double* pool_fap, int32_t pool_cap,
+                          int64_t* base_idx, double* base_freq, int32_t* n_base_out);
 
 /*
  * fredec_trig_averages -- the trigonometric averages behind the gradient and Fisher matrix of the

@@ -5,7 +5,8 @@ CUDA path.  Each function follows the passage it cites, in the paper's order and
 Pins (tests/test_phase1_pins.py; subset_fits: tests/test_subset_pins.py; refine:
 tests/test_refine_pins.py): zstat against (N_H/2) ln(l_base/l_alt) with both l from QR fits;
 T_eff against the closed form for evenly spaced, equally weighted times; fap1 against hand values;
-phase 1 on constructed series whose outcome the rules fix.  The coefficient A~_1 of eq. 13 and the
+phase 1 on constructed series whose outcome the rules fix (with refine_base: two OFF-grid sinusoids must
+give a base of exactly two frequencies, each at the true value).  The coefficient A~_1 of eq. 13 and the
 readings P1-P4 are not fixed by the paper: parity unpinned for those.
 """
 from __future__ import annotations
@@ -68,8 +69,17 @@ def _grid_frequency(f0: float, df: float, k: int) -> float:
 
 
 def phase1(t, x, w, f0, df, K, fap0=0.05, fap1_thr=0.1, A1=1.0, max_base=10, k_peaks=32, pool_cap=None,
-           threads: int = 0):
-    """PAPER.md:199-210 (section 4.2).  Returns dict(pool_idx, pool_z, pool_fap, base_idx)."""
+           threads: int = 0, refine_base: bool = False, refine_iter: int = 20, refine_tol: float = 1e-9):
+    """PAPER.md:199-210 (section 4.2).  Returns dict(pool_idx, pool_z, pool_fap, base_idx, base_freqs).
+
+    refine_base (reading P5): "adding to the base model the frequency corresponding to
+    the largest peak" taken as the paper's own fit of such a model -- after the peak's grid
+    frequency has joined the base, ALL base frequencies are refitted together by the local multifrequency
+    fit of eq. 17 (`refine` below), and the next residual periodogram uses the refitted,
+    off-grid frequencies.  Without it a signal up to df/2 off the grid leaves a residue that re-enters the
+    base at the neighbouring grid point.  base_idx stays the grid index of each iteration's top peak;
+    base_freqs are the frequencies the base ends with.  If the local fit fails (singular normal equations)
+    the unrefined frequencies are kept for that iteration."""
     t = np.asarray(t, dtype=np.float64)
     N = t.shape[0]
     pool_cap = max(1, N // 10) if pool_cap is None else pool_cap
@@ -98,11 +108,16 @@ def phase1(t, x, w, f0, df, K, fap0=0.05, fap1_thr=0.1, A1=1.0, max_base=10, k_p
                     pool[i] = (float(z[j]), float(fap[j]))
         base_idx.append(int(idx[0]))                            # "adding to the base model the frequency
         base_f.append(_grid_frequency(f0, df, int(idx[0])))     #  corresponding to the largest peak"
+        if refine_base and N >= 3 * len(base_f) + 2:
+            try:
+                base_f = [float(f) for f in refine(t, x, w, base_f, max_iter=refine_iter, tol=refine_tol)[0]]
+            except np.linalg.LinAlgError:
+                pass
     entries = sorted(pool.items(), key=lambda kv: (kv[1][1], kv[0]))
     entries = entries[:min(N // 10, pool_cap)]
     return {"pool_idx": np.array([e[0] for e in entries], dtype=np.int64),
             "pool_z": np.array([e[1][0] for e in entries]), "pool_fap": np.array([e[1][1] for e in entries]),
-            "base_idx": np.array(base_idx, dtype=np.int64)}
+            "base_idx": np.array(base_idx, dtype=np.int64), "base_freqs": np.array(base_f, dtype=np.float64)}
 
 
 def subset_fits(t, x, w, freqs, tau: float = 1e-10, masks=None, return_pivots: bool = False):

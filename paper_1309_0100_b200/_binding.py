@@ -38,6 +38,8 @@ SIGNATURES = {
     "fredec_bandwidth": (C.c_int, [_P, _P, _I64, _F64, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
     "fredec_phase1": (C.c_int, [_P, _P, _P, _I64, _F64, _F64, _I64, _F64, _F64, _F64, _I32, _I32,
                                 _P, _P, _P, _I32, _P, C.POINTER(C.c_int32)]),
+    "fredec_phase1_refined": (C.c_int, [_P, _P, _P, _I64, _F64, _F64, _I64, _F64, _F64, _F64, _I32, _I32, _I32, _F64,
+                                        _P, _P, _P, _I32, _P, _P, C.POINTER(C.c_int32)]),
     "fredec_trig_averages": (C.c_int, [_P, _P, _P, _I64, _P, _I64, _P]),
     "fredec_subset_fits": (C.c_int, [_P, _P, _P, _I64, _P, _I32, _P]),
     "fredec_refine": (C.c_int, [_P, _P, _P, _I64, _P, _I32, _I32, _F64, C.POINTER(C.c_double),
@@ -293,22 +295,36 @@ def fredec_bandwidth(t, w, f_max):
     return te.value, W.value
 
 
-def fredec_phase1(t, x, w, f0, df, K, fap0=0.05, fap1=0.1, A1=1.0, max_base=10, k_peaks=32, pool_cap=None):
+def fredec_phase1(t, x, w, f0, df, K, fap0=0.05, fap1=0.1, A1=1.0, max_base=10, k_peaks=32, pool_cap=None,
+                  refine_base=False, refine_iter=20, refine_tol=1e-9):
     """Phase 1 of FREDEC (preliminary scan): returns a dict with the candidate pool (grid indices,
-    statistic, FAP; sorted by FAP) and the base frequencies' grid indices in the order found."""
+    statistic, FAP; sorted by FAP) and the base frequencies' grid indices in the order found.
+    refine_base: fredec_phase1_refined (the base frequencies are refitted after every addition); the dict
+    then also holds base_freqs, the frequencies the base ends with."""
     N = int(t.shape[-1])
     pool_cap = max(1, N // 10) if pool_cap is None else int(pool_cap)
     pool_idx = np.empty(pool_cap, dtype=np.int64)
     pool_z, pool_fap = np.empty(pool_cap), np.empty(pool_cap)
     base_idx = np.empty(int(max_base), dtype=np.int64)
+    base_freq = np.empty(int(max_base))
     n_base = C.c_int32(0)
     (pt, kt), (px, kx), (pw, kw) = map(_ptr, (t, x, w))
-    n = _check(lib().fredec_phase1(pt, px, pw, N, float(f0), float(df), int(K), float(fap0), float(fap1),
-                                   float(A1), int(max_base), int(k_peaks), pool_idx.ctypes.data,
-                                   pool_z.ctypes.data, pool_fap.ctypes.data, pool_cap, base_idx.ctypes.data,
-                                   C.byref(n_base)), "fredec_phase1")
-    return {"pool_idx": pool_idx[:n].copy(), "pool_z": pool_z[:n].copy(), "pool_fap": pool_fap[:n].copy(),
-            "base_idx": base_idx[:n_base.value].copy()}
+    if refine_base:
+        n = _check(lib().fredec_phase1_refined(
+            pt, px, pw, N, float(f0), float(df), int(K), float(fap0), float(fap1), float(A1), int(max_base),
+            int(k_peaks), int(refine_iter), float(refine_tol), pool_idx.ctypes.data, pool_z.ctypes.data,
+            pool_fap.ctypes.data, pool_cap, base_idx.ctypes.data, base_freq.ctypes.data, C.byref(n_base)),
+            "fredec_phase1_refined")
+    else:
+        n = _check(lib().fredec_phase1(pt, px, pw, N, float(f0), float(df), int(K), float(fap0), float(fap1),
+                                       float(A1), int(max_base), int(k_peaks), pool_idx.ctypes.data,
+                                       pool_z.ctypes.data, pool_fap.ctypes.data, pool_cap, base_idx.ctypes.data,
+                                       C.byref(n_base)), "fredec_phase1")
+    out = {"pool_idx": pool_idx[:n].copy(), "pool_z": pool_z[:n].copy(), "pool_fap": pool_fap[:n].copy(),
+           "base_idx": base_idx[:n_base.value].copy()}
+    if refine_base:
+        out["base_freqs"] = base_freq[:n_base.value].copy()
+    return out
 
 
 def fredec_trig_averages(t, x, w, freqs, out=None):

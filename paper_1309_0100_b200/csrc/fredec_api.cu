@@ -752,12 +752,18 @@ int fredec_bandwidth(const double* t, const double* w, int64_t N, double f_max, 
     return FREDEC_OK;
 }
 
-int fredec_phase1(const double* t, const double* x, const double* w, int64_t N, double f0, double df, int64_t K,
-                  double fap0, double fap1, double A1, int32_t max_base, int32_t k_peaks, int64_t* pool_idx,
-                  double* pool_z, double* pool_fap, int32_t pool_cap, int64_t* base_idx, int32_t* n_base_out)
+// Phase 1 in both forms.  refine == false: fredec_phase1 (the peak's GRID frequency joins the base, which
+// grows in place).  refine == true: fredec_phase1_refined (after every addition all base frequencies are
+// refitted by the device Gauss-Newton of fredec_refine and the base is rebuilt from the refitted values).
+static int phase1_impl(const double* t, const double* x, const double* w, int64_t N, double f0, double df, int64_t K,
+                       double fap0, double fap1, double A1, int32_t max_base, int32_t k_peaks, int64_t* pool_idx,
+                       double* pool_z, double* pool_fap, int32_t pool_cap, int64_t* base_idx, int32_t* n_base_out,
+                       bool refine, int32_t refine_iter, double refine_tol, double* base_freq_out)
 {
     if (!t || !x || !w || !pool_idx || !pool_z || !pool_fap || !base_idx || !n_base_out) return FREDEC_EINVAL;
     if (N < 4 || pool_cap < 1 || max_base < 1 || 2 * max_base + 1 > FREDEC_D_MAX) return FREDEC_EINVAL;
+    if (refine && (max_base > 25 || refine_iter < 0 || !(refine_tol > 0.0) || !base_freq_out || on_device(base_freq_out)))
+        return FREDEC_EINVAL;
     if (!(fap0 > 0.0) || !(fap1 <= 1.0) || !(fap0 <= fap1) || !(A1 > 0.0) || !std::isfinite(A1)) return FREDEC_EINVAL;
     int rc = check_grid_args(f0, df, K);
     if (rc) return rc;
@@ -777,7 +783,7 @@ int fredec_phase1(const double* t, const double* x, const double* w, int64_t N, 
     const double f_max = f0 + df * (double)(K - 1);
     const double W = f_max * bw[0];  // W = f_max T_eff
 
-    CK(g.p1_base.reserve((size_t)N * 8));
+    CK(g.p1_base.reserve((size_t)(refine ? 2 * max_base + 1 : 1) * N * 8));
     // the orthonormal base grows in place from iteration to iteration: room for the last one now
     CK(g.psi.reserve((size_t)(2 * max_base + 1) * N * 8));
     CK(g.xt.reserve((size_t)N * 8));
@@ -804,6 +810,12 @@ int fredec_phase1(const double* t, const double* x, const double* w, int64_t N, 
         if (m == 0) {
             // the constant alone: orthogonalisation from scratch (the prep kernel)
             CK(launch_sin_base(dt, N, g.p1_freq.as<double>(), 0, g.p1_base.as<double>(), st));
+            rc1 = do_scan(dt, dx, dw, 1, N, g.p1_base.as<double>(), d, f0, df, K, g.p1_z.as<double>(), k_peaks,
+                          g.p1_idx.as<int64_t>(), true, true);
+        } else if (refine) {
+            // every base frequency moved in the refit: constant + m sinusoids rebuilt and orthogonalised anew
+            CK(cudaMemcpyAsync(g.p1_freq.as<double>(), base_f.data(), (size_t)m * 8, cudaMemcpyHostToDevice, st));
+            CK(launch_sin_base(dt, N, g.p1_freq.as<double>(), m, g.p1_base.as<double>(), st));
             rc1 = do_scan(dt, dx, dw, 1, N, g.p1_base.as<double>(), d, f0, df, K, g.p1_z.as<double>(), k_peaks,
                           g.p1_idx.as<int64_t>(), true, true);
         } else {
@@ -846,7 +858,19 @@ int fredec_phase1(const double* t, const double* x, const double* w, int64_t N, 
         base_idx[m] = idx[0];
         base_f.push_back(std::fma((double)idx[0], df, f0));
         *n_base_out = m + 1;
+        if (refine && N >= 3 * (int64_t)(m + 1) + 2) {
+            // PAPER.md:177-185 (eq. 17): joint local fit of all base frequencies, the new one included; when
+            // the normal equations are singular the unrefined values stay (reading P5)
+            std::vector<double> fr(base_f);
+            double l_loc = 0.0;
+            const int rr = fredec_refine(dt, dx, dw, N, fr.data(), m + 1, refine_iter, refine_tol, &l_loc, nullptr);
+            launches += g.launches;
+            if (rr == FREDEC_OK) base_f.swap(fr);
+            else if (rr != FREDEC_ESINGULAR) return rr;
+        }
     }
+    if (base_freq_out)
+        for (size_t i = 0; i < base_f.size(); ++i) base_freq_out[i] = base_f[i];
     std::sort(pool.begin(), pool.end(), [](const PoolEntry& a, const PoolEntry& b) {
         return a.fap < b.fap || (a.fap == b.fap && a.idx < b.idx);
     });
@@ -860,6 +884,24 @@ int fredec_phase1(const double* t, const double* x, const double* w, int64_t N, 
     }
     g.launches = launches;
     return (int)n;
+}
+
+int fredec_phase1(const double* t, const double* x, const double* w, int64_t N, double f0, double df, int64_t K,
+                  double fap0, double fap1, double A1, int32_t max_base, int32_t k_peaks, int64_t* pool_idx,
+                  double* pool_z, double* pool_fap, int32_t pool_cap, int64_t* base_idx, int32_t* n_base_out)
+{
+    return phase1_impl(t, x, w, N, f0, df, K, fap0, fap1, A1, max_base, k_peaks, pool_idx, pool_z, pool_fap, pool_cap,
+                       base_idx, n_base_out, false, 0, 0.0, nullptr);
+}
+
+int fredec_phase1_refined(const double* t, const double* x, const double* w, int64_t N, double f0, double df,
+                          int64_t K, double fap0, double fap1, double A1, int32_t max_base, int32_t k_peaks,
+                          int32_t refine_iter, double refine_tol, int64_t* pool_idx, double* pool_z,
+                          double* pool_fap, int32_t pool_cap, int64_t* base_idx, double* base_freq,
+                          int32_t* n_base_out)
+{
+    return phase1_impl(t, x, w, N, f0, df, K, fap0, fap1, A1, max_base, k_peaks, pool_idx, pool_z, pool_fap, pool_cap,
+                       base_idx, n_base_out, true, refine_iter, refine_tol, base_freq);
 }
 
 int fredec_trig_averages(const double* t, const double* x, const double* w, int64_t N, const double* freqs, int64_t M,

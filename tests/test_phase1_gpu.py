@@ -10,6 +10,7 @@ import pytest
 from paper_1309_0100_b200 import inputs
 
 pytestmark = pytest.mark.gpu
+TWO_PI = 2.0 * np.pi
 
 
 @pytest.fixture(scope="module")
@@ -82,6 +83,74 @@ def test_phase1_rv_like_series(fr, p1):
     import torch
     rd = fr.fredec_phase1(*[torch.from_numpy(a).cuda() for a in (t, x, w)], wl.f0, wl.df, wl.K, **kw)
     _assert_phase1_equal(rd, r)
+
+
+def _assert_refined_equal(r, ref, T_eff, tol):
+    """Both sides stop their Gauss-Newton when the last step is below tol cycles over T_eff, so the refitted
+    frequencies agree to a few tol; the periodograms that follow depend smoothly on them: the discrete
+    outcome (which peaks, in which order) must be identical, the statistics agree to 1e-7 relative and the
+    FAPs, proportional to e^-z, to 1e-7 z."""
+    assert r["base_idx"].tolist() == ref["base_idx"].tolist()
+    assert r["pool_idx"].tolist() == ref["pool_idx"].tolist()
+    assert np.max(np.abs(r["base_freqs"] - ref["base_freqs"])) * T_eff <= 10 * tol
+    assert np.all(np.abs(r["pool_z"] - ref["pool_z"]) <= 1e-7 * np.abs(ref["pool_z"]))
+    assert np.all(np.abs(r["pool_fap"] - ref["pool_fap"]) <= (1e-7 * (1.0 + ref["pool_z"])) * ref["pool_fap"] + 1e-300)
+
+
+def test_phase1_refined_two_off_grid_sinusoids(fr, p1):
+    """fredec_phase1_refined (PAPER.md:201 with the fit of PAPER.md:177-185): two sinusoids between grid points
+    and almost no noise -- the base ends with exactly the two true frequencies, as the oracle's does, and
+    the grid-only mode on the same series does not."""
+    rng = np.random.Generator(np.random.PCG64(8))
+    N, K, f0, df, noise = 150, 4000, 0.002, 0.00025, 1e-7
+    t = np.sort(rng.uniform(0.0, 200.0, N))
+    fa, fb = f0 + 1213.41 * df, f0 + 2790.47 * df
+    x = 3.0 * np.sin(TWO_PI * fa * t + 0.3) + 1.2 * np.cos(TWO_PI * fb * t) + 0.7 + noise * rng.standard_normal(N)
+    w = np.full(N, 1.0 / noise ** 2)
+    T_eff, _ = p1.bandwidth(t, w, 1.0)
+    tol = 1e-11
+    ref = p1.phase1(t, x, w, f0, df, K, fap0=0.01, fap1_thr=0.02, max_base=6, k_peaks=20, refine_base=True,
+                    refine_iter=30, refine_tol=tol)
+    r = fr.fredec_phase1(t, x, w, f0, df, K, fap0=0.01, fap1=0.02, max_base=6, k_peaks=20, refine_base=True,
+                         refine_iter=30, refine_tol=tol)
+    assert r["base_idx"].tolist() == [1213, 2790]
+    assert np.max(np.abs(r["base_freqs"] - np.array([fa, fb]))) <= 1e-6 / (t.max() - t.min())
+    _assert_refined_equal(r, ref, T_eff, tol)
+    grid_only = fr.fredec_phase1(t, x, w, f0, df, K, fap0=0.01, fap1=0.02, max_base=6, k_peaks=20)
+    assert len(grid_only["base_idx"]) > 2 and "base_freqs" not in grid_only
+
+
+def test_phase1_refined_rv_like_series_full_config2(fr, p1):
+    """Config 2 in full (N = 1000, K = 80 000): with the refit the base holds the five injected signals once
+    each (the grid-only mode enters two of them twice, at neighbouring grid points); pool, base and refitted
+    frequencies equal the oracle's; host and device pointers agree bit for bit."""
+    import torch
+    wl = inputs.config(2)
+    t, x, w, _ = wl.series(0)
+    T_eff, _ = p1.bandwidth(t, w, 1.0)
+    tol = 1e-11
+    ref = p1.phase1(t, x, w, wl.f0, wl.df, wl.K, max_base=10, k_peaks=32, refine_base=True, refine_iter=30,
+                    refine_tol=tol)
+    r = fr.fredec_phase1(t, x, w, wl.f0, wl.df, wl.K, max_base=10, k_peaks=32, refine_base=True, refine_iter=30,
+                         refine_tol=tol)
+    _assert_refined_equal(r, ref, T_eff, tol)
+    bi = np.sort(r["base_idx"])
+    assert len(bi) == 5 and np.all(np.diff(bi) > 1)
+    true_f = 1.0 / np.array(inputs.RV_PERIODS)
+    assert all(np.min(np.abs(true_f - f)) <= 0.1 / (t.max() - t.min()) for f in r["base_freqs"])
+    rd = fr.fredec_phase1(*[torch.from_numpy(a).cuda() for a in (t, x, w)], wl.f0, wl.df, wl.K, max_base=10,
+                          k_peaks=32, refine_base=True, refine_iter=30, refine_tol=tol)
+    for key in ("base_idx", "pool_idx", "base_freqs", "pool_z", "pool_fap"):
+        assert np.array_equal(rd[key], r[key]), key
+    grid_only = fr.fredec_phase1(t, x, w, wl.f0, wl.df, wl.K, max_base=10, k_peaks=32)
+    assert np.any(np.diff(np.sort(grid_only["base_idx"])) == 1)
+    # max_base cuts the loop; a refit needs N >= 3 m + 2 observations and max_base <= 25
+    r2 = fr.fredec_phase1(t, x, w, wl.f0, wl.df, wl.K, max_base=2, k_peaks=32, refine_base=True)
+    assert r2["base_idx"].tolist() == r["base_idx"][:2].tolist() and r2["base_freqs"].shape == (2,)
+    for bad in (dict(max_base=26), dict(refine_tol=0.0), dict(refine_iter=-1)):
+        with pytest.raises(fr.FredecError) as e:
+            fr.fredec_phase1(t, x, w, wl.f0, wl.df, wl.K, refine_base=True, **bad)
+        assert e.value.code == fr.FREDEC_EINVAL
 
 
 def test_phase1_tiny_config_and_noise(fr, p1):

@@ -7,6 +7,7 @@ Pin                                         | catches
 closed-form T_eff for even spacing          | variance normalisation, factor 4 pi, weights
 hand values of W e^-z sqrt z                | exponent sign, power of z, cap at 1
 constructed series for phase 1              | stop rule, base order, half-height rule, N/10 cap
+off-grid sinusoids, refine_base             | a refit that is skipped, applied to the wrong entry, or not fed back
 """
 import numpy as np
 import pytest
@@ -107,6 +108,53 @@ def test_phase1_finds_two_grid_sinusoids_then_stops(p1):
     # max_base cuts the SLICK loop short
     r1 = p1.phase1(t, x, w, f0, df, K, fap0=0.01, fap1_thr=0.02, max_base=1, k_peaks=20)
     assert r1["base_idx"].tolist() == [k1]
+
+
+def _two_off_grid_sinusoids(N=150, K=4000, noise=1e-7, seed=8):
+    rng = np.random.Generator(np.random.PCG64(seed))
+    t = np.sort(rng.uniform(0.0, 200.0, N))
+    f0, df = 0.002, 0.00025
+    fa, fb = f0 + 1213.41 * df, f0 + 2790.47 * df    # 0.41 and 0.47 of a grid step off the grid
+    x = (3.0 * np.sin(TWO_PI * fa * t + 0.3) + 1.2 * np.cos(TWO_PI * fb * t) + 0.7
+         + noise * rng.standard_normal(N))
+    return t, x, np.full(N, 1.0 / noise ** 2), f0, df, K, fa, fb
+
+
+def test_phase1_refined_base_holds_each_off_grid_signal_once(p1):
+    """PAPER.md:201 + :177-185 (reading P5): two sinusoids BETWEEN grid points, almost no noise.  With the
+    base refitted after every addition the base ends with exactly the two true frequencies (to 1e-6 / T; the
+    noise allows ~1e-8 / T) and the third periodogram is noise.  The grid-only mode, on the same series, keeps
+    finding the residue the mis-tuned base leaves behind -- which is why the refit matters."""
+    t, x, w, f0, df, K, fa, fb = _two_off_grid_sinusoids()
+    T = t.max() - t.min()
+    r = p1.phase1(t, x, w, f0, df, K, fap0=0.01, fap1_thr=0.02, max_base=6, k_peaks=20, refine_base=True)
+    assert r["base_idx"].tolist() == [1213, 2790]                 # the peaks' grid points, strongest first
+    assert r["base_freqs"].shape == (2,)
+    assert np.max(np.abs(r["base_freqs"] - np.array([fa, fb]))) <= 1e-6 / T
+    assert {1213, 2790} <= set(r["pool_idx"].tolist())
+    grid_only = p1.phase1(t, x, w, f0, df, K, fap0=0.01, fap1_thr=0.02, max_base=6, k_peaks=20)
+    assert len(grid_only["base_idx"]) > 2
+    assert np.array_equal(grid_only["base_freqs"], f0 + df * grid_only["base_idx"])
+    # one iteration only: the refit of a single frequency against the second, unmodelled signal
+    r1 = p1.phase1(t, x, w, f0, df, K, fap0=0.01, fap1_thr=0.02, max_base=1, k_peaks=20, refine_base=True)
+    assert r1["base_idx"].tolist() == [1213] and abs(r1["base_freqs"][0] - fa) <= 0.05 / T
+
+
+def test_phase1_refined_on_the_rv_like_series(p1):
+    """The config-2 series carries five sinusoids (inputs.RV_PERIODS).  Grid-only phase 1 enters two of them
+    twice, at neighbouring grid points; with the refit the base holds five frequencies, no two of them
+    adjacent on the grid, each within a tenth of a cycle over the span of an injected one."""
+    wl = inputs.config(2)
+    t, x, w, _ = wl.series(0)
+    T = t.max() - t.min()
+    r = p1.phase1(t, x, w, wl.f0, wl.df, wl.K, max_base=10, k_peaks=32, refine_base=True)
+    bi = np.sort(r["base_idx"])
+    assert len(bi) == 5 and np.all(np.diff(bi) > 1)
+    true_f = 1.0 / np.array(inputs.RV_PERIODS)
+    for f in r["base_freqs"]:
+        assert np.min(np.abs(true_f - f)) <= 0.1 / T
+    grid_only = p1.phase1(t, x, w, wl.f0, wl.df, wl.K, max_base=10, k_peaks=32)
+    assert np.any(np.diff(np.sort(grid_only["base_idx"])) == 1)   # the duplicates the refit removes
 
 
 def test_phase1_half_height_rule_and_pool_cap(p1):
