@@ -279,6 +279,34 @@ def run_phase1(fr, inputs, dev, with_oracle: bool):
     return rec
 
 
+def run_topk_noalloc(fr, dev, stream, z_dev, k):
+    """fredec_topk_noalloc (fixed built-in scratch, one launch, no allocation) beside fredec_topk (library
+    workspace, two launches) on the periodogram the timed steps left in z_dev: same indices, device time of
+    each by CUDA events over 20 calls."""
+    import torch
+    idx = torch.empty(k, dtype=torch.int64, device=dev)
+    cnt = torch.empty(1, dtype=torch.int32, device=dev)
+    ref, ref_count = fr.fredec_topk(z_dev, k)
+    fr.fredec_topk_noalloc(z_dev, k, idx, cnt, stream=stream)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    out = {"K": int(z_dev.shape[0]), "k": int(k), "scratch_bytes": fr.fredec_topk_noalloc_scratch_bytes(),
+           "equal_to_fredec_topk": bool(torch.equal(idx, ref)) and int(cnt.item()) == ref_count}
+    fr.fredec_set_timing(False)
+    try:
+        for name, call in (("noalloc_ms", lambda: fr.fredec_topk_noalloc(z_dev, k, idx, cnt, stream=stream)),
+                           ("fredec_topk_ms", lambda: fr.fredec_topk(z_dev, k, idx_out=idx))):
+            a.record(stream)
+            for _ in range(20):
+                call()
+            b.record(stream)
+            torch.cuda.synchronize()
+            out[name] = a.elapsed_time(b) / 20
+    finally:
+        fr.fredec_set_timing(True)
+    return out
+
+
 def main_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -497,6 +525,7 @@ def main_ours(args):
     if world == 1 and not args.no_small_configs:
         line["configs"] = run_small_configs(fr, inputs, dev, stream, peak_nominal, with_oracle=cpu is not None)
         line["phase1"] = run_phase1(fr, inputs, dev, with_oracle=cpu is not None)
+        line["topk_noalloc"] = run_topk_noalloc(fr, dev, stream, z_dev, wl.topk)
     if multi:
         line["multi_series"] = multi
     if cpu:

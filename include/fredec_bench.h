@@ -1,9 +1,10 @@
 /*
- * fredec_bench.h -- measurement tooling exported by libfredec_b200.so beside the product ABI of
- * fredec.h.  Nothing here is part of the method (arXiv:1309.0100); these calls exist so that bench.py
+ * fredec_bench.h -- measurement tooling, exported by libfredec_bench.so (built beside the product library
+ * libfredec_b200.so, which exports fredec.h and nothing else; only bench.py loads it).  Nothing here is part
+ * of the method (arXiv:1309.0100); these calls exist so that bench.py
  * can state the FP64 roofline denominator of the box it runs on (MEASURED_PEAKS.json has no FP64
  * figure) and what a scalar FP64 instruction costs next to the scan kernel's FP64 MMA stream.
- * Conventions (status codes, stream, synchronous return) as in fredec.h.
+ * Status codes as in fredec.h; the probes run on the default stream and return when they have completed.
  */
 #ifndef FREDEC_BENCH_H
 #define FREDEC_BENCH_H
@@ -16,7 +17,7 @@ extern "C" {
 
 /*
  * fredec_bench_fp64 -- runs one register-resident FP64 probe on all SMs and times it with CUDA events
- * on the library's stream (one warm-up launch first).
+ * on the default stream (one warm-up launch first).
  *   mode 0     DFMA only, 2048 threads per SM, 8 independent chains per thread: the FP64 FMA peak.
  *              iters = FMAs per chain (>= 1024); tflops_out counts 2 flops per FMA.
  *   mode >= 1  a DMMA (mma.sync.m8n8k4.f64) loop, one CTA of 8 MMA warps per SM, optionally mixed with

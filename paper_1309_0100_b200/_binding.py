@@ -52,15 +52,21 @@ SIGNATURES = {
     "fredec_pending": (C.c_int, []),
     "fredec_last_timing": (C.c_int, [C.POINTER(C.c_double)]),
     "fredec_last_launches": (C.c_int, []),
-    "fredec_bench_fp64": (C.c_int, [_I32, _I64, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
-    "fredec_bench_fp64_name": (C.c_char_p, [_I32]),
     "fredec_shutdown": (C.c_int, []),
     "fredec_strerror": (C.c_char_p, [C.c_int]),
     "fredec_last_cuda_error": (C.c_int, []),
     "fredec_version": (C.c_int, []),
 }
 
+# include/fredec_bench.h: the FP64 roofline probes live in a library of their own (bench.py only)
+BENCH_LIB_PATH = os.path.join(_HERE, "libfredec_bench.so")
+BENCH_SIGNATURES = {
+    "fredec_bench_fp64": (C.c_int, [_I32, _I64, C.POINTER(C.c_double), C.POINTER(C.c_double)]),
+    "fredec_bench_fp64_name": (C.c_char_p, [_I32]),
+}
+
 _lib = None
+_bench_lib = None
 
 
 class FredecError(RuntimeError):
@@ -84,6 +90,21 @@ def lib():
             fn.argtypes = args
         _lib = L
     return _lib
+
+
+def bench_lib():
+    """Loads libfredec_bench.so (measurement probes); raises if it has not been built."""
+    global _bench_lib
+    if _bench_lib is None:
+        if not os.path.exists(BENCH_LIB_PATH):
+            raise RuntimeError(f"{BENCH_LIB_PATH} is missing: build it with `python -m paper_1309_0100_b200.build`")
+        L = C.CDLL(BENCH_LIB_PATH)
+        for name, (res, args) in BENCH_SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype = res
+            fn.argtypes = args
+        _bench_lib = L
+    return _bench_lib
 
 
 def _check(rc: int, where: str) -> int:
@@ -395,12 +416,12 @@ def fredec_bench_fp64(mode: int = 0, iters: int = 1 << 16):
     """(TFLOP/s, ms) of an FP64 roofline probe (include/fredec_bench.h): mode 0 = DFMA only (the FP64
     FMA peak), modes >= 1 = DMMA loops, see fredec_bench_fp64_name."""
     tf, ms = C.c_double(), C.c_double()
-    _check(lib().fredec_bench_fp64(int(mode), int(iters), C.byref(tf), C.byref(ms)), "fredec_bench_fp64")
+    _check(bench_lib().fredec_bench_fp64(int(mode), int(iters), C.byref(tf), C.byref(ms)), "fredec_bench_fp64")
     return tf.value, ms.value
 
 
 def fredec_bench_fp64_name(mode: int):
-    name = lib().fredec_bench_fp64_name(int(mode))
+    name = bench_lib().fredec_bench_fp64_name(int(mode))
     return None if name is None else name.decode()
 
 

@@ -1,5 +1,5 @@
-"""Build libfredec_b200.so (the C-ABI library of include/fredec.h) in-tree with nvcc for
-sm_100a.  `python -m paper_1309_0100_b200.build [--force]`.  nvcc cross-compiles without a GPU.
+"""Build libfredec_b200.so (the C-ABI library of include/fredec.h) and libfredec_bench.so (the FP64 roofline
+probes of include/fredec_bench.h, for bench.py) in-tree with nvcc for sm_100a.  `python -m paper_1309_0100_b200.build [--force]`.  nvcc cross-compiles without a GPU.
 
 Measurement builds: `python -m paper_1309_0100_b200.build --variant NAME -DMACRO[=V] ...` compiles the
 same sources with extra macros (the FREDEC_EXP_* switches documented where they appear in csrc/) into
@@ -17,7 +17,10 @@ ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 OBJ = os.path.join(PKG, "build")
 LIB = os.path.join(PKG, "libfredec_b200.so")
-SOURCES = ["fredec_api.cu", "prep_kernel.cu", "scan_mma_kernel.cu", "topk_kernel.cu", "topk_noalloc.cu", "peak_kernel.cu", "stat_kernel.cu", "trig_kernel.cu", "subset_kernel.cu", "refine_kernel.cu"]
+SOURCES = ["fredec_api.cu", "prep_kernel.cu", "scan_mma_kernel.cu", "topk_kernel.cu", "topk_noalloc.cu", "stat_kernel.cu", "trig_kernel.cu", "subset_kernel.cu", "refine_kernel.cu"]
+# the FP64 roofline probes of include/fredec_bench.h: a library of their own, loaded by bench.py only
+BENCH_LIB = os.path.join(PKG, "libfredec_bench.so")
+BENCH_SOURCES = ["bench_api.cu", "peak_kernel.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
 
@@ -63,6 +66,17 @@ def build(force: bool = False, verbose: bool = False, variant: str = "", defines
     objs = [os.path.join(obj_dir, s.replace(".cu", ".o")) for s in SOURCES]
     if jobs or not os.path.exists(lib_path):
         run([nvcc, "-shared", "-o", lib_path, *objs, "-gencode", "arch=compute_100a,code=sm_100a"])
+    if not variant:
+        bench_objs, stale = [], False
+        for src in BENCH_SOURCES:
+            s = os.path.join(CSRC, src)
+            o = os.path.join(obj_dir, src.replace(".cu", ".o"))
+            bench_objs.append(o)
+            if force or not os.path.exists(o) or os.path.getmtime(o) < max(os.path.getmtime(s), hdr):
+                run([nvcc, *NVCC_FLAGS, "-c", s, "-o", o])
+                stale = True
+        if stale or not os.path.exists(BENCH_LIB):
+            run([nvcc, "-shared", "-o", BENCH_LIB, *bench_objs, "-gencode", "arch=compute_100a,code=sm_100a"])
     return lib_path
 
 

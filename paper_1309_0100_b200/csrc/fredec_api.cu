@@ -10,8 +10,6 @@
 #include <cuda_runtime.h>
 
 #include "fredec.h"
-#include "fredec_bench.h"
-#include "peak_kernel.cuh"
 #include "prep_kernel.cuh"
 #include "scan_mma_kernel.cuh"
 #include "refine_kernel.cuh"
@@ -1100,41 +1098,6 @@ int fredec_set_timing(int32_t enable)
 }
 
 int fredec_last_launches(void) { return g.launches; }
-
-int fredec_bench_fp64(int32_t mode, int64_t iters, double* tflops_out, double* ms_out)
-{
-    if (!tflops_out || mode < 0 || mode > dmma_probe_count()) return FREDEC_EINVAL;
-    if (mode == 0 ? iters < 1024 : (iters < 64 || iters % 4 != 0)) return FREDEC_EINVAL;
-    int rc = ensure_ready();
-    if (rc) return rc;
-    CK(g.sink.reserve(64));
-    cudaStream_t st = g.stream;
-    double flops;
-    if (mode == 0) {
-        const int blocks = g.sm_count * 8;  // 2048 threads per SM
-        CK(launch_dfma(1024, blocks, g.sink.as<double>(), st));  // warm-up
-        CK(cudaEventRecord(g.ev[0], st));
-        CK(launch_dfma(iters, blocks, g.sink.as<double>(), st));
-        flops = dfma_flops(iters, blocks);
-    } else {
-        CK(launch_dmma_probe(mode - 1, 64, g.sm_count, g.sink.as<double>(), st));
-        CK(cudaEventRecord(g.ev[0], st));
-        CK(launch_dmma_probe(mode - 1, iters, g.sm_count, g.sink.as<double>(), st));
-        flops = dmma_probe_flops(iters, g.sm_count);
-    }
-    CK(cudaEventRecord(g.ev[1], st));
-    CK(cudaStreamSynchronize(st));
-    const double ms = ev_ms(0, 1);
-    *tflops_out = ms > 0.0 ? flops / (ms * 1e-3) * 1e-12 : 0.0;
-    if (ms_out) *ms_out = ms;
-    return FREDEC_OK;
-}
-
-const char* fredec_bench_fp64_name(int32_t mode)
-{
-    if (mode == 0) return "dfma only, 2048 threads per SM";
-    return dmma_probe_name(mode - 1);
-}
 
 int fredec_shutdown(void)
 {

@@ -19,27 +19,33 @@ def fr():
     return fr
 
 
-def declared_symbols():
-    """Every function any header under include/ declares (fredec.h: the product ABI; fredec_bench.h: the
-    measurement probes)."""
-    names = set()
-    inc = os.path.join(ROOT, "include")
-    for h in sorted(os.listdir(inc)):
-        if h.endswith(".h"):
-            text = re.sub(r"/\*.*?\*/", "", open(os.path.join(inc, h)).read(), flags=re.S)
-            names |= set(re.findall(r"\b(fredec_[a-z0-9_]+)\s*\(", text))
-    return sorted(names)
+def declared_symbols(header):
+    """Every function a header under include/ declares."""
+    text = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", header)).read(), flags=re.S)
+    return sorted(set(re.findall(r"\b(fredec_[a-z0-9_]+)\s*\(", text)))
 
 
 def test_header_symbols_are_exported_and_bound(fr):
+    """fredec.h <-> libfredec_b200.so <-> the binding, name for name; the measurement probes of
+    fredec_bench.h live in libfredec_bench.so and the product library does not export them."""
+    import subprocess
     from paper_1309_0100_b200 import _binding
-    names = declared_symbols()
+    names = declared_symbols("fredec.h")
     assert len(names) >= 14
     L = ctypes.CDLL(_binding.LIB_PATH)
     for n in names:
         assert hasattr(L, n), f"{n} declared in fredec.h but not exported"
         assert n in _binding.SIGNATURES, f"{n} has no ctypes signature in the binding"
     assert sorted(_binding.SIGNATURES) == names
+    exported = subprocess.run(["nm", "-D", "--defined-only", _binding.LIB_PATH], capture_output=True, text=True).stdout
+    exported = sorted(set(re.findall(r"\b(fredec_[a-z0-9_]+)$", exported, flags=re.M)))
+    assert exported == names, "the product library exports exactly what fredec.h declares"
+    bench_names = declared_symbols("fredec_bench.h")
+    assert sorted(_binding.BENCH_SIGNATURES) == bench_names and len(bench_names) == 2
+    B = ctypes.CDLL(_binding.BENCH_LIB_PATH)
+    for n in bench_names:
+        assert hasattr(B, n) and not hasattr(L, n)
+    assert fr.fredec_bench_fp64_name(0) and fr.fredec_bench_fp64_name(10_000) is None
 
 
 def test_library_targets_sm_100a(fr):
